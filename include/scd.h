@@ -1,0 +1,189 @@
+/* scd.h -- C ABI of the B200-native SCD KV state codec (arxiv/paper_2606_07684).
+ *
+ * Semantic Cache Distillation replaces raw KV transmission between a producer model
+ * M_A and a weight-mismatched consumer M_B of the same architecture by per-layer
+ * low-rank "semantic codes".  This library is the data-parallel hot
+ * path of that method on one B200 (sm_100a):
+ *
+ *   scd_plan          static routing table + artifact store   (Alg.1 :174)
+ *   scd_encode        producer:  Z_K = deRoPE(K_A) W_enc,K ; Z_V = V_A W_enc,V   (Eq. 5, Eq. 8 :145)
+ *                                Z_H = x_norm,A W_enc,H on PATCH layers          (Eq. 10, :165)
+ *   scd_reuse_decode  consumer:  K_B = RoPE(Z_K W_dec,K) ; V_B = Z_V W_dec,V     (Eq. 9 :150, :152)
+ *   scd_patch         consumer:  H^ = g_theta(Z_H) ; K^ = RoPE(H^ W_k) ; V^ = H^ W_v   (Eq. 11 :171, Eq. 12 :190-193)
+ *
+ * Results are written straight into a paged KV cache (the "cache container" of
+ * PAPER.md:610, here a pool of `block_size`-token pages; build extension).
+ *
+ * Conventions
+ *  - extern "C", plain pointers and sizes; no exceptions, no global mutable state.
+ *  - Unless a comment says HOST, every data pointer is a DEVICE pointer that the caller
+ *    owns ("borrowed"); the library never frees or keeps it past the call, except that
+ *    scd_plan keeps its own repacked copies of the artifacts.
+ *  - Hot calls (scd_encode / scd_reuse_decode / scd_patch) enqueue kernels on `stream`
+ *    (a cudaStream_t passed as void*) and return without synchronising or allocating.
+ *  - Argument / shape / alignment problems are detected on the host and returned as a
+ *    status before anything is enqueued; scd_last_error() gives a thread-local message.
+ *  - Layer indices are 0-based.  All matrices are row-major.
+ *  - Alignment: every base pointer 16 B (128 B recommended), code buffer 128 B; strides
+ *    of bf16 tensors multiples of 8 elements (TMA needs 16-B pitches).
+ *  - Writes: exactly the slots { page_table[b][t/bs]*bs + t%bs : 0 <= t < len_b } of the
+ *    addressed layers' pools, nothing else.
+ */
+#ifndef SCD_H_
+#define SCD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SCD_MAX_LAYERS 128
+
+typedef struct scd_plan scd_plan_t;          /* opaque; immutable after creation */
+
+typedef enum {
+  SCD_OK = 0,
+  SCD_E_ARG = 1,          /* NULL / out-of-range argument                         */
+  SCD_E_SHAPE = 2,        /* inconsistent shapes                                  */
+  SCD_E_UNSUPPORTED = 3,  /* legal but not implemented combination */
+  SCD_E_ALIGN = 4,        /* pointer / stride alignment                            */
+  SCD_E_WORKSPACE = 5,    /* workspace too small                                   */
+  SCD_E_CUDA = 6,         /* CUDA runtime / driver error                           */
+  SCD_E_NOMEM = 7
+} scd_status_t;
+
+typedef enum { SCD_F32 = 0, SCD_BF16 = 1, SCD_E4M3_ROWSCALE = 2 } scd_dtype_t;
+typedef enum { SCD_REUSE = 0, SCD_PATCH = 1 } scd_kind_t;
+typedef enum { SCD_BRANCH_K = 0, SCD_BRANCH_V = 1, SCD_BRANCH_H = 2 } scd_branch_t;
+/* HALF = HF rotate_half, pairs (j, j + d_h/2); INTERLEAVED pairs (2j, 2j+1). */
+typedef enum { SCD_ROPE_HALF = 0, SCD_ROPE_INTERLEAVED = 1 } scd_rope_t;
+typedef enum { SCD_ACT_IDENTITY = 0, SCD_ACT_SILU = 1 } scd_act_t;
+/* NORM_NONE is the paper-literal Eq. 11-12; NORM_RMS: h = gamma * u / sqrt(mean(u^2)+eps). */
+typedef enum { SCD_NORM_NONE = 0, SCD_NORM_RMS = 1 } scd_norm_t;
+
+/* Model-pair geometry; producer and consumer share the architecture. */
+typedef struct {
+  int32_t n_layers;        /* 1 .. SCD_MAX_LAYERS                                        */
+  int32_t d_model;
+  int32_t n_kv_heads;
+  int32_t head_dim;        /* 32, 64 or 128                                              */
+  int32_t block_size;      /* tokens per KV page (16)                                    */
+  int32_t max_position;    /* RoPE table length; every position id must be < this        */
+  int32_t state_dtype;     /* scd_dtype_t F32 | BF16: K/V/hidden, artifacts, pools       */
+  int32_t code_dtype;      /* scd_dtype_t F32 | BF16 | E4M3_ROWSCALE                     */
+  double  rope_theta_producer;
+  double  rope_theta_consumer;
+  int32_t rope_style;      /* scd_rope_t                                                 */
+  int32_t k_is_roped;      /* producer K is post-RoPE: encode applies deRoPE (Eq. 5)     */
+  int32_t rope_on_reuse_k; /* decode re-applies RoPE to K; 0 for tests    */
+  int32_t patch_act;       /* scd_act_t                                                  */
+  int32_t patch_norm;      /* scd_norm_t                                                 */
+  float   rms_eps;
+} scd_model_desc_t;
+
+/* One per layer.  Artifacts are in state_dtype unless typed float. NULL means "absent"
+ * (mean / bias = 0).  REUSE fields are read when kind == SCD_REUSE, PATCH fields when
+ * kind == SCD_PATCH.  D = n_kv_heads * head_dim. */
+typedef struct {
+  int32_t kind;                      /* scd_kind_t                                       */
+  int32_t r_k, r_v;                  /* REUSE ranks, independent          */
+  const void *enc_k, *enc_v;         /* [D, r]  producer encoders  (Eq. 7-8)             */
+  const void *dec_k, *dec_v;         /* [r, D]  consumer decoders  (Eq. 6, 9)            */
+  const float *mean_src_k, *mean_src_v;   /* [D] subtracted before encode, or NULL       */
+  const float *mean_dst_k, *mean_dst_v;   /* [D] added after decode, or NULL             */
+  int32_t r_h, d_aligner;            /* PATCH: code rank r_H, aligner hidden width d_a   */
+  const void *enc_h;                 /* [d_model, r_h]                   */
+  const float *mean_src_h;           /* [d_model] or NULL                                */
+  const void *w1, *b1;               /* [r_h, d_a], [d_a]     aligner layer 1 (Eq. 11)   */
+  const void *w2, *b2;               /* [d_a, d_model], [d_model]  aligner layer 2       */
+  const void *norm_gamma;            /* [d_model] consumer RMSNorm weight (NORM_RMS)     */
+  const void *w_k, *w_v;             /* [D, d_model]  HF layout [out, in]  (Eq. 12)      */
+  const void *b_k, *b_v;             /* [D] or NULL                                      */
+} scd_layer_desc_t;
+
+/* A ragged batch.  Packed row n = cu_seqlens[b] + t; position id = pos_offset[b] + t. */
+typedef struct {
+  int32_t n_seqs, total_tokens, max_seqlen, max_pages_per_seq;
+  const int32_t *cu_seqlens;         /* [n_seqs + 1]                                     */
+  const int32_t *page_table;         /* [n_seqs, max_pages_per_seq] block ids, unused -1 */
+  const int32_t *pos_offset;         /* [n_seqs] first position id, or NULL (= 0)        */
+  int32_t max_pos_offset;            /* HOST upper bound on pos_offset[] (0 if NULL)     */
+} scd_batch_t;
+
+/* Producer states.  k, v, h are HOST arrays of n_layers DEVICE pointers. */
+typedef struct {
+  const void *const *k;              /* [n_layers] -> [total_tokens, H_kv, d_h]; REUSE layers read */
+  const void *const *v;
+  const void *const *h;              /* [n_layers] -> [total_tokens, d_model]; PATCH layers read   */
+  int64_t kv_token_stride, kv_head_stride, h_token_stride;   /* in elements              */
+} scd_src_t;
+
+/* Consumer paged pool.  k_pool, v_pool are HOST arrays of n_layers DEVICE pointers, each
+ * -> [n_blocks, block_size, H_kv, d_h] in state_dtype. */
+typedef struct {
+  void *const *k_pool;
+  void *const *v_pool;
+  int32_t n_blocks;
+} scd_paged_kv_t;
+
+/* Create a plan: validates, classifies layers (REUSE | PATCH), copies and repacks the
+ * artifacts into plan-owned device memory (transposes to K-major, folds gamma into
+ * W_k|W_v, precomputes c = mu_src W_enc in fp64 and the RoPE tables), builds the TMA
+ * descriptors of the plan-owned operands.  Work is enqueued on `stream`; the caller may
+ * free its artifact buffers after synchronising it.  *out is NULL on failure. */
+scd_status_t scd_plan(const scd_model_desc_t* model, const scd_layer_desc_t* layers /* HOST [n_layers] */,
+                      void* stream, scd_plan_t** out);
+scd_status_t scd_plan_destroy(scd_plan_t* plan);
+
+/* Sizes for a call over `total_tokens` packed rows: code buffer bytes (with padding),
+ * workspace bytes scd_patch needs, and the transport payload |Z| of Eq. 3 (
+ * codes + e4m3 scales, no padding).  Any out pointer may be NULL. */
+scd_status_t scd_plan_query(const scd_plan_t* plan, int32_t total_tokens,
+                            size_t* code_bytes, size_t* patch_workspace_bytes, size_t* payload_bytes);
+
+/* Where the codes of (layer, branch) live in the code buffer: [total_tokens, rank]
+ * row-major in code_dtype at `offset`; for E4M3_ROWSCALE the fp32 row scales
+ * [total_tokens] at `scale_offset` (else (size_t)-1).  REUSE layers have branches K, V;
+ * PATCH layers branch H; anything else is SCD_E_ARG. */
+scd_status_t scd_plan_code_segment(const scd_plan_t* plan, int32_t layer, int32_t branch,
+                                   int32_t total_tokens, size_t* offset, size_t* scale_offset,
+                                   int32_t* rank);
+
+/* The same layout arithmetic as a pure HOST function (no plan, no CUDA): used to size
+ * buffers before a plan exists and by the CPU tests.  Only kind, r_k, r_v, r_h of each
+ * layer are read.  layer < 0 skips the per-segment outputs. */
+scd_status_t scd_code_layout(const scd_model_desc_t* model, const scd_layer_desc_t* layers,
+                             int32_t total_tokens, int32_t layer, int32_t branch,
+                             size_t* offset, size_t* scale_offset, int32_t* rank,
+                             size_t* code_bytes, size_t* payload_bytes);
+
+/* Producer side (Alg. 1 :176-180).  Reads K, V of every REUSE layer and H of every PATCH
+ * layer, writes every code segment of `codes` (size >= code_bytes). */
+scd_status_t scd_encode(const scd_plan_t* plan, const scd_batch_t* batch, const scd_src_t* src,
+                        void* codes, void* stream);
+
+/* Consumer side, REUSE layers only (Alg. 1 :182-184): codes x basis (+ mean), RoPE on K,
+ * cast, paged write. */
+scd_status_t scd_reuse_decode(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
+                              const scd_paged_kv_t* kv, void* stream);
+
+/* Consumer side, PATCH layers only (Eq. 11-12): aligner -> RMS-consistent scaling ->
+ * [W_k | W_v] -> RoPE on K -> paged write.  `workspace` >= patch_workspace_bytes. */
+scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
+                       const scd_paged_kv_t* kv, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Number of kernels the last hot call on this thread enqueued (for bench accounting). */
+int32_t scd_last_launch_count(void);
+
+/* Thread-local message for the last non-OK status returned on this thread ("" if none). */
+const char* scd_last_error(void);
+
+/* Library version string. */
+const char* scd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SCD_H_ */
