@@ -1,0 +1,382 @@
+#!/usr/bin/env python
+"""bench.py -- SCD KV state codec on B200: one "step" = one pass of the whole hot path
+(scd_encode -> scd_reuse_decode -> scd_patch, every row of SURVEY.md 8(a)) over one batch of
+synthetic input.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  `value` = packed tokens whose K/V were rebuilt for all layers
+per second of device time (CUDA events around the three C-ABI calls, L2 flushed between calls
+outside the events, max over ranks).  `e2e` = the same with HOST buffers: pinned producer
+states copied H2D, the three calls, the reconstructed pools copied D2H, all inside the timed
+region.  `roofline` = the dominant kernel of the step, timed live with CUDA events on its
+launching stream (scd_profile_* hooks).  `cpu_baseline` / `--impl reference` = the fp64 oracle
+timed on the box's host cores on a bounded row sample.  Multi-GPU: the path has no exchange
+step, so N ranks run N independent replicas ("replicas only") -- weak scaling.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "reconstructed KV tokens/s (REUSE+PATCH hybrid cache, encode->reuse_decode->patch)"
+UNIT = "tokens/s"
+KERNEL_NAMES = {100: "tc_gemm<codes,plain> (encode V/H)", 101: "tc_gemm<codes,derope> (encode K)",
+                110: "tc_gemm<paged_kv> (reuse decode / patch GEMM-3)", 120: "tc_gemm<aligner_in> (patch GEMM-1)",
+                130: "tc_gemm<aligner_out> (patch GEMM-2)"}
+
+
+# ------------------------------------------------------------------------------ helpers
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"],
+                "bf16_tflops_sustained": d.get("bf16_tflops_sustained", d["bf16_tflops"]), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({n for r in self.rows if len(r) >= 6 for n, v in zip(names, r[2:6]) if v == "Active"})
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def workload_costs(cfg, T):
+    """Algorithmic bytes / FLOPs per call (stated in DESIGN.md)."""
+    cb = {0: 4, 1: 2, 2: 1}[cfg.code_dtype]
+    sb = 4 if cfg.code_dtype == 2 else 0
+    ob = 4 if cfg.state_dtype == 0 else 2
+    D, d, d_a, r = cfg.D, cfg.d_model, cfg.d_a, cfg.rank
+    P = len(cfg.patch_layers)
+    R = cfg.n_layers - P
+    c = {}
+    c["reuse_bytes"] = R * T * (2 * (r * cb + sb) + 2 * D * ob)
+    c["reuse_flops"] = R * T * 4 * r * D
+    c["encode_bytes"] = R * T * (2 * D * ob + 2 * (r * cb + sb)) + P * T * (d * ob + r * cb + sb)
+    c["encode_flops"] = R * T * 4 * D * r + P * T * 2 * d * r
+    c["patch_flops"] = P * T * 2 * (r * d_a + d_a * d + 2 * d * D)
+    c["patch_bytes"] = P * T * (r * cb + sb + 2 * D * ob)
+    c["kv_bytes_written"] = cfg.n_layers * T * 2 * D * ob
+    c["gemm2_flops_per_launch"] = T * 2 * d_a * d
+    c["gemm3_flops_per_launch"] = T * 2 * d * 2 * D
+    c["gemm1_flops_per_launch"] = T * 2 * r * d_a
+    return c
+
+
+# ------------------------------------------------------------------------------ oracle arm
+def oracle_sample_rate(cfg, n_rows: int, seed: int = 0):
+    """Time the oracle (as it stands) on `n_rows` sampled rows of the workload, all layers:
+    encode + pack + reuse_decode + patch.  Returns (rows per second, seconds, threads)."""
+    import numpy as np
+    import torch
+    from oracle import scd_oracle as O
+    from paper_2606_07684_b200 import workloads as W
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"] or [1])
+    except Exception:
+        threads = os.cpu_count() or 1
+    n64 = lambda t: None if t is None else t.double().numpy()
+    om = O.Model(n_layers=cfg.n_layers, d_model=cfg.d_model, n_kv_heads=cfg.n_kv_heads, head_dim=cfg.head_dim,
+                 block_size=cfg.block_size, rope_theta_producer=cfg.rope_theta, rope_theta_consumer=cfg.rope_theta,
+                 code_dtype=cfg.code_dtype, rms_eps=cfg.rms_eps)
+    pos = np.random.default_rng(seed).integers(0, max(1, max(cfg.seqlens or (2048,))), n_rows)
+    elapsed = 0.0
+    for l in range(cfg.n_layers):
+        a = W.make_layer_artifacts(cfg, l, "cpu", cal_rows=1024)      # untimed: calibration artifacts
+        if a.kind == W.REUSE:
+            lay = O.Layer(O.REUSE, enc_k=n64(a.enc_k), enc_v=n64(a.enc_v), dec_k=n64(a.dec_k), dec_v=n64(a.dec_v),
+                          mean_src_k=n64(a.mean_k), mean_src_v=n64(a.mean_v), mean_dst_k=n64(a.mean_k), mean_dst_v=n64(a.mean_v))
+            k, v = n64(W.make_state(cfg, l, 0, n_rows, "cpu")), n64(W.make_state(cfg, l, 1, n_rows, "cpu"))
+            t0 = time.perf_counter()
+            qk, sk = O.pack_codes(O.encode_k(om, lay, k, pos), om.code_dtype)
+            qv, sv = O.pack_codes(O.encode_v(om, lay, v), om.code_dtype)
+            O.reuse_decode_layer(om, lay, O.unpack_codes(qk, sk, om.code_dtype), O.unpack_codes(qv, sv, om.code_dtype), pos)
+            elapsed += time.perf_counter() - t0
+        else:
+            lay = O.Layer(O.PATCH, enc_h=n64(a.enc_h), mean_src_h=n64(a.mean_h), w1=n64(a.w1), b1=n64(a.b1), w2=n64(a.w2),
+                          norm_gamma=n64(a.gamma), w_k=n64(a.w_k), w_v=n64(a.w_v))
+            h = n64(W.make_state(cfg, l, 2, n_rows, "cpu"))
+            t0 = time.perf_counter()
+            qh, sh = O.pack_codes(O.encode_h(om, lay, h), om.code_dtype)
+            O.patch_layer(om, lay, O.unpack_codes(qh, sh, om.code_dtype), pos)
+            elapsed += time.perf_counter() - t0
+    return n_rows / elapsed, elapsed, threads
+
+
+def run_reference(args, cfg):
+    """--impl reference: the oracle on the host cores, each step a bounded row sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_rows = args.ref_rows
+    for _ in range(args.warmup):
+        oracle_sample_rate(cfg, min(n_rows, 16))
+    times, threads = [], 1
+    for s in range(args.steps):
+        rate, sec, threads = oracle_sample_rate(cfg, n_rows, seed=s)
+        times.append(sec)
+    sec = sum(times) / len(times)
+    val = n_rows / sec
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "sample": f"{n_rows} seeded rows x all {cfg.n_layers} layers per step"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
+                             "sample": f"{n_rows} rows x {cfg.n_layers} layers (encode+reuse_decode+patch), numpy fp64"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------ our arm
+def run_ours(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_07684_b200 import binding as B
+    from paper_2606_07684_b200.harness import CodecProblem
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = torch.device(f"cuda:{local}")
+    torch.cuda.set_device(dev)
+
+    prob = CodecProblem(cfg, dev)
+    T = prob.T
+    k, v, h = prob.make_sources()          # content-space states stand in for the post-RoPE cache
+    prob.alloc_pools()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def one_step(timed):
+        """encode -> decode -> patch with L2 flushed before each call; returns per-call ms."""
+        evs = []
+        launches = 0
+        for fn in (lambda: prob.encode(k, v, h), prob.reuse_decode, prob.patch):
+            flush.fill_(1)
+            a, b = ev(), ev()
+            a.record(stream)
+            launches += fn()
+            b.record(stream)
+            evs.append((a, b))
+        return evs, launches
+
+    for _ in range(max(args.warmup, 3)):
+        one_step(False)
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    t_wall = time.perf_counter()
+    all_evs, launches = [], 0
+    for _ in range(args.steps):
+        evs, n = one_step(True)
+        all_evs.append(evs)
+        launches += n
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    per_call = [[a.elapsed_time(b) for a, b in evs] for evs in all_evs]
+    enc_ms, dec_ms, pat_ms = (sum(c[i] for c in per_call) / len(per_call) for i in range(3))
+    step_ms = enc_ms + dec_ms + pat_ms
+
+    # ---- per-kernel times (events inside the library, same stream), for the roofline ----
+    B.profile_enable(True)
+    for _ in range(min(args.steps, 5)):
+        one_step(False)
+    torch.cuda.synchronize()
+    recs = B.profile_fetch()
+    B.profile_enable(False)
+    by_kernel = {}
+    for kid, ms in recs:
+        by_kernel.setdefault(kid, []).append(ms)
+
+    # ---- e2e: host buffers in, host buffers out ----
+    e2e = None
+    if not args.no_e2e:
+        srcs = [t for t in (k + v + h) if t is not None]
+        pools = [p for p in (prob.k_pool + prob.v_pool)]
+        host_in = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True).copy_(t) for t in srcs]
+        host_out = [torch.empty(p.shape, dtype=p.dtype, pin_memory=True) for p in pools]
+        h2d = sum(t.numel() * t.element_size() for t in srcs)
+        d2h = sum(p.numel() * p.element_size() for p in pools)
+
+        def e2e_step():
+            for dst, src in zip(srcs, host_in):
+                dst.copy_(src, non_blocking=True)
+            prob.encode(k, v, h); prob.reuse_decode(); prob.patch()
+            for dst, src in zip(host_out, pools):
+                dst.copy_(src, non_blocking=True)
+
+        e2e_step()
+        barrier()
+        a, b = ev(), ev()
+        n_e2e = max(2, min(args.steps, 5))
+        a.record(stream)
+        for _ in range(n_e2e):
+            e2e_step()
+        b.record(stream)
+        barrier()
+        e2e_ms = a.elapsed_time(b) / n_e2e
+        e2e = {"ms": e2e_ms, "h2d": h2d, "d2h": d2h}
+    clocks = sampler.stop() if sampler else None
+
+    # ---- max over ranks ----
+    vals = torch.tensor([step_ms, enc_ms, dec_ms, pat_ms, e2e["ms"] if e2e else 0.0], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+    step_ms, enc_ms, dec_ms, pat_ms, e2e_ms = vals.tolist()
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = load_peaks()
+    costs = workload_costs(cfg, T)
+    tokens = T * world
+    value = tokens / (step_ms * 1e-3)
+
+    # dominant kernel of the step = largest total time over the profiled passes
+    tot = {kid: sum(v_) for kid, v_ in by_kernel.items()}
+    dom = max(tot, key=tot.get) if tot else None
+    rooflines = {}
+    n_prof = max(1, min(args.steps, 5))
+    for kid, ts in by_kernel.items():
+        avg_ms = sum(ts) / len(ts)
+        per_pass = len(ts) / n_prof
+        if kid == 110:      # paged-KV kernel: reuse decode launches (HBM) and patch GEMM-3 launches (tensor) differ
+            n_dec = 1 if cfg.n_layers > len(cfg.patch_layers) else 0
+            # launches arrive in call order: decode first, then one GEMM-3 per patch layer
+            dec_ts = [t for i, t in enumerate(ts) if n_dec and i % int(per_pass) == 0]
+            g3_ts = [t for i, t in enumerate(ts) if not (n_dec and i % int(per_pass) == 0)]
+            if dec_ts:
+                a_ms = sum(dec_ts) / len(dec_ts)
+                ach = costs["reuse_bytes"] / (a_ms * 1e-3) / 1e9
+                rooflines["reuse_decode"] = {"kernel": KERNEL_NAMES[kid], "bound": "hbm", "achieved": ach,
+                                             "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                                             "traffic": None, "ms": a_ms, "share_of_step": a_ms / step_ms}
+            if g3_ts:
+                a_ms = sum(g3_ts) / len(g3_ts)
+                ach = costs["gemm3_flops_per_launch"] / (a_ms * 1e-3) / 1e12
+                rooflines["patch_gemm3"] = {"kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach,
+                                            "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                                            "frac": ach / peaks["bf16_tflops_sustained"], "traffic": None, "ms": a_ms,
+                                            "share_of_step": a_ms * len(cfg.patch_layers) / step_ms}
+        elif kid in (120, 130):
+            fl = costs["gemm1_flops_per_launch"] if kid == 120 else costs["gemm2_flops_per_launch"]
+            ach = fl / (avg_ms * 1e-3) / 1e12
+            rooflines["patch_gemm1" if kid == 120 else "patch_gemm2"] = {
+                "kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"],
+                "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"], "traffic": None, "ms": avg_ms,
+                "share_of_step": avg_ms * len(cfg.patch_layers) / step_ms}
+        elif kid in (100, 101):
+            pass
+    if enc_ms > 0:
+        ach = costs["encode_bytes"] / (enc_ms * 1e-3) / 1e9
+        rooflines["encode_call"] = {"kernel": "scd_encode (all launches)", "bound": "hbm", "achieved": ach,
+                                    "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                                    "traffic": None, "ms": enc_ms, "share_of_step": enc_ms / step_ms}
+    dom_key = max(rooflines, key=lambda n: rooflines[n]["share_of_step"]) if rooflines else None
+    roofline = dict(rooflines[dom_key]) if dom_key else None
+    if roofline:
+        roofline["name"] = dom_key
+        roofline["peak_source"] = peaks["source"] + (" sustained bf16" if roofline["bound"] == "tensor" else " copy")
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if cfg.state_dtype == 1 else "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "tokens": T, "layers": cfg.n_layers, "patch_layers": list(cfg.patch_layers),
+                   "rank": cfg.rank, "code_dtype": {0: "f32", 1: "bf16", 2: "e4m3+f32 rowscale"}[cfg.code_dtype],
+                   "l2": "flushed (256 MiB fill) before every C-ABI call, outside the events; inputs 2.2 GB >> L2",
+                   "parallelism": "replicas only" if world > 1 else "1 gpu"},
+        "stages_ms": {"encode": enc_ms, "reuse_decode": dec_ms, "patch": pat_ms},
+        "kv_tokens_per_s_reuse_plus_patch": tokens / ((dec_ms + pat_ms) * 1e-3),
+        "kv_gbs_written": costs["kv_bytes_written"] * world / ((dec_ms + pat_ms) * 1e-3) / 1e9,
+        "reuse_decode_tokens_per_s": tokens / (dec_ms * 1e-3) if dec_ms else None,
+        "gpu_launches": launches, "wall_s_timed_region": t_wall,
+        "clocks": clocks, "roofline": roofline, "rooflines": rooflines,
+    }
+    if e2e:
+        line["e2e"] = {"value": tokens / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
+                       "d2h_bytes_per_step": e2e["d2h"], "ms_per_step": e2e_ms}
+    if world == 1 and not args.no_cpu_baseline:
+        rate, sec, threads = oracle_sample_rate(cfg, args.ref_rows)
+        line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"{args.ref_rows} seeded rows x all {cfg.n_layers} layers "
+                                          f"(encode+reuse_decode+patch), numpy fp64, {sec:.1f} s"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="llama3_8b_8k")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-rows", type=int, default=256)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    from paper_2606_07684_b200 import workloads as W
+    cfg = W.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+        return
+    import __graft_entry__ as ge
+    ge.build()
+    run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

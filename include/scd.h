@@ -177,6 +177,16 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
 /* Number of kernels the last hot call on this thread enqueued (for bench accounting). */
 int32_t scd_last_launch_count(void);
 
+/* Per-kernel timing for measurement harnesses.  While enabled (on != 0) every kernel a hot
+ * call on this thread enqueues is bracketed by CUDA events on the caller's stream.
+ * scd_profile_fetch synchronises those events and returns, for up to `max` launches since
+ * the last fetch, the elapsed milliseconds and a kernel id
+ * (100*path + 10*epilogue + a_mode; path 0 = SIMT, 1 = tcgen05; epilogue 0 codes, 1 paged KV,
+ * 2 aligner-in, 3 aligner-out; a_mode 0 plain, 1 deRoPE, 2 codes).  Returns the number of
+ * launches recorded (may exceed max).  Off by default; adds two event records per launch. */
+scd_status_t scd_profile_enable(int32_t on);
+int32_t scd_profile_fetch(float* ms /* HOST [max] */, int32_t* kernel_id /* HOST [max] */, int32_t max);
+
 /* Thread-local message for the last non-OK status returned on this thread ("" if none). */
 const char* scd_last_error(void);
 

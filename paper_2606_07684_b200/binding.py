@@ -31,7 +31,8 @@ NO_SCALE = C.c_size_t(-1).value
 
 # every symbol include/scd.h declares
 EXPORTS = ["scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
-           "scd_encode", "scd_reuse_decode", "scd_patch", "scd_last_launch_count", "scd_last_error", "scd_version"]
+           "scd_encode", "scd_reuse_decode", "scd_patch", "scd_last_launch_count", "scd_profile_enable",
+           "scd_profile_fetch", "scd_last_error", "scd_version"]
 
 
 class ModelDesc(C.Structure):
@@ -94,6 +95,10 @@ def _load() -> C.CDLL:
                  "scd_encode", "scd_reuse_decode", "scd_patch"):
         getattr(lib, name).restype = C.c_int
     lib.scd_last_launch_count.restype = C.c_int32
+    lib.scd_profile_enable.argtypes = [i32]
+    lib.scd_profile_enable.restype = C.c_int
+    lib.scd_profile_fetch.argtypes = [C.POINTER(C.c_float), pi32, i32]
+    lib.scd_profile_fetch.restype = C.c_int32
     lib.scd_last_error.restype = C.c_char_p
     lib.scd_version.restype = C.c_char_p
     return lib
@@ -237,6 +242,18 @@ def scd_patch(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequenc
     _check(lib.scd_patch(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _ptr(workspace), ws_bytes,
                          _stream_ptr(stream)))
     return lib.scd_last_launch_count()
+
+
+def profile_enable(on: bool) -> None:
+    _check(lib.scd_profile_enable(int(on)))
+
+
+def profile_fetch(max_launches: int = 4096):
+    """[(kernel_id, ms)] for every launch since the last fetch (synchronises their events)."""
+    ms = (C.c_float * max_launches)()
+    ids = (C.c_int32 * max_launches)()
+    n = min(lib.scd_profile_fetch(ms, ids, max_launches), max_launches)
+    return [(ids[i], ms[i]) for i in range(n)]
 
 
 def version() -> str:

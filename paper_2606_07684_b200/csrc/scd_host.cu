@@ -24,6 +24,24 @@ scd_status_t fail(scd_status_t st, const char* fmt, ...) {
 }
 void count_launch() { ++g_launches; }
 
+struct ProfRec { cudaEvent_t a, b; int id; };
+static thread_local bool g_prof_on = false;
+static thread_local std::vector<ProfRec>* g_prof = nullptr;
+void prof_begin(cudaStream_t s) {
+  if (!g_prof_on) return;
+  if (!g_prof) g_prof = new std::vector<ProfRec>();
+  ProfRec r{};
+  cudaEventCreate(&r.a);
+  cudaEventCreate(&r.b);
+  cudaEventRecord(r.a, s);
+  g_prof->push_back(r);
+}
+void prof_end(cudaStream_t s, int kernel_id) {
+  if (!g_prof_on || !g_prof || g_prof->empty()) return;
+  g_prof->back().id = kernel_id;
+  cudaEventRecord(g_prof->back().b, s);
+}
+
 #define SCD_CUDA(expr)                                                                          \
   do {                                                                                          \
     cudaError_t _e = (expr);                                                                    \
@@ -286,6 +304,29 @@ extern "C" {
 const char* scd_last_error(void) { return g_err; }
 int32_t scd_last_launch_count(void) { return g_launches; }
 const char* scd_version(void) { return "scd-b200 0.1 (sm_100a)"; }
+
+scd_status_t scd_profile_enable(int32_t on) {
+  g_prof_on = on != 0;
+  return SCD_OK;
+}
+int32_t scd_profile_fetch(float* ms, int32_t* kernel_id, int32_t max) {
+  if (!g_prof) return 0;
+  int32_t n = (int32_t)g_prof->size();
+  for (int32_t i = 0; i < n; ++i) {
+    ProfRec& r = (*g_prof)[i];
+    float t = 0.0f;
+    cudaEventSynchronize(r.b);
+    cudaEventElapsedTime(&t, r.a, r.b);
+    if (i < max) {
+      if (ms) ms[i] = t;
+      if (kernel_id) kernel_id[i] = r.id;
+    }
+    cudaEventDestroy(r.a);
+    cudaEventDestroy(r.b);
+  }
+  g_prof->clear();
+  return n;
+}
 
 scd_status_t scd_code_layout(const scd_model_desc_t* model, const scd_layer_desc_t* layers, int32_t total_tokens,
                              int32_t layer, int32_t branch, size_t* offset, size_t* scale_offset, int32_t* rank,

@@ -121,6 +121,9 @@ namespace scd {
 // ---- error plumbing (scd_host.cu) -------------------------------------------------
 scd_status_t fail(scd_status_t st, const char* fmt, ...);
 void count_launch();
+// profiling hooks (scd_profile_enable): bracket one launch with events on `s`
+void prof_begin(cudaStream_t s);
+void prof_end(cudaStream_t s, int kernel_id);
 
 // ---- layout (scd_host.cu) ---------------------------------------------------------
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }

@@ -213,7 +213,9 @@ cudaError_t launch(const GemmSeg& g, int epi, int a_mode, int code_dtype, const 
                                            (int)smem);                                                        \
       if (e != cudaSuccess) return e;                                                                         \
     }                                                                                                         \
+    prof_begin(s);                                                                                            \
     simt_gemm_kernel<TS, E><<<grid, NT, smem, s>>>(g, a_mode, code_dtype, batch, rope, ntpb);                 \
+    prof_end(s, 10 * E + a_mode);                                                                             \
     break;                                                                                                    \
   }
   switch (epi) {

@@ -578,7 +578,9 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
     configured = smem;
   }
   const int grid = std::min(total, p->sm_count);
+  prof_begin(s);
   tc_gemm_kernel<EPI, AMODE><<<grid, AMODE == A_DEROPE ? 384 : 256, smem, s>>>(P);
+  prof_end(s, 100 + 10 * EPI + AMODE);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));
   count_launch();
