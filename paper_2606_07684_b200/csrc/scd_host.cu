@@ -195,6 +195,9 @@ static bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 // ---------------------------------------------------------------------------------
 // plan construction
 // ---------------------------------------------------------------------------------
+// fp32 epilogue vectors are read with 16-byte loads up to one tile (256 columns) past N
+static const size_t kVecPad = 256 * sizeof(float);
+
 template <typename T>
 static scd_status_t dev_alloc(scd_plan_t* p, T** out, size_t bytes) {
   void* ptr = nullptr;
@@ -202,6 +205,7 @@ static scd_status_t dev_alloc(scd_plan_t* p, T** out, size_t bytes) {
   if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? SCD_E_NOMEM : SCD_E_CUDA, "cudaMalloc(%zu): %s",
                                     bytes, cudaGetErrorString(e));
   p->allocs.push_back(ptr);
+  cudaMemset(ptr, 0, bytes ? bytes : 16);
   *out = (T*)ptr;
   return SCD_OK;
 }
@@ -243,7 +247,7 @@ static scd_status_t build_plan(scd_plan_t* p, const scd_layer_desc_t* layers, cu
       sp.layer = l; sp.branch = br; sp.rank = r; sp.width = width; sp.seg_index = (int)p->segs.size();
       if ((st = dev_alloc(p, &sp.enc_t, (size_t)r * width * es)) != SCD_OK) return st;
       SCD_CUDA(prep_transpose(enc, sp.enc_t, width, r, sd, s));            // [width, r] -> [r, width]
-      if ((st = dev_alloc(p, &sp.enc_c, (size_t)r * 4)) != SCD_OK) return st;
+      if ((st = dev_alloc(p, &sp.enc_c, (size_t)r * 4 + kVecPad)) != SCD_OK) return st;
       SCD_CUDA(prep_mean_proj(mu_s, enc, sp.enc_c, width, r, sd, s));
       if (mu_s) {
         if ((st = dev_alloc(p, &sp.mean_src, (size_t)width * 4)) != SCD_OK) return st;
@@ -252,7 +256,7 @@ static scd_status_t build_plan(scd_plan_t* p, const scd_layer_desc_t* layers, cu
       if (dec) {
         if ((st = dev_alloc(p, &sp.dec_t, (size_t)D * r * es)) != SCD_OK) return st;
         SCD_CUDA(prep_transpose(dec, sp.dec_t, r, D, sd, s));              // [r, D] -> [D, r]
-        if ((st = dev_alloc(p, &sp.mean_dst, (size_t)D * 4)) != SCD_OK) return st;
+        if ((st = dev_alloc(p, &sp.mean_dst, (size_t)D * 4 + kVecPad)) != SCD_OK) return st;
         SCD_CUDA(prep_copy_f32(mu_d, sp.mean_dst, D, s));
       }
       p->seg_of[(size_t)l * 3 + br] = sp.seg_index;
@@ -270,17 +274,17 @@ static scd_status_t build_plan(scd_plan_t* p, const scd_layer_desc_t* layers, cu
     pp.layer = l; pp.r_h = L.r_h; pp.d_a = L.d_aligner; pp.h_seg = p->seg_of[(size_t)l * 3 + SCD_BRANCH_H];
     if ((st = dev_alloc(p, &pp.w1_t, (size_t)pp.d_a * pp.r_h * es)) != SCD_OK) return st;
     SCD_CUDA(prep_transpose(L.w1, pp.w1_t, pp.r_h, pp.d_a, sd, s));        // [r_h, d_a] -> [d_a, r_h]
-    if ((st = dev_alloc(p, &pp.b1, (size_t)pp.d_a * 4)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.b1, (size_t)pp.d_a * 4 + kVecPad)) != SCD_OK) return st;
     SCD_CUDA(prep_to_f32(L.b1, pp.b1, pp.d_a, sd, s));
     if ((st = dev_alloc(p, &pp.w2_t, (size_t)d * pp.d_a * es)) != SCD_OK) return st;
     SCD_CUDA(prep_transpose(L.w2, pp.w2_t, pp.d_a, d, sd, s));             // [d_a, d] -> [d, d_a]
-    if ((st = dev_alloc(p, &pp.b2, (size_t)d * 4)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.b2, (size_t)d * 4 + kVecPad)) != SCD_OK) return st;
     SCD_CUDA(prep_to_f32(L.b2, pp.b2, d, sd, s));
     if ((st = dev_alloc(p, &pp.wkv, (size_t)2 * D * d * es)) != SCD_OK) return st;
     const void* gamma = m.patch_norm == SCD_NORM_RMS ? L.norm_gamma : nullptr;
     SCD_CUDA(prep_fold_gamma(L.w_k, gamma, pp.wkv, D, d, sd, s));
     SCD_CUDA(prep_fold_gamma(L.w_v, gamma, (char*)pp.wkv + (size_t)D * d * es, D, d, sd, s));
-    if ((st = dev_alloc(p, &pp.bkv, (size_t)2 * D * 4)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.bkv, (size_t)2 * D * 4 + kVecPad)) != SCD_OK) return st;
     SCD_CUDA(prep_to_f32(L.b_k, pp.bkv, D, sd, s));
     SCD_CUDA(prep_to_f32(L.b_v, pp.bkv + D, D, sd, s));
     p->patches.push_back(pp);

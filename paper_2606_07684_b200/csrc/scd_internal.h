@@ -110,10 +110,8 @@ struct scd_plan {
   bool use_tc = false;                                // bf16 state -> tcgen05 kernels
   bool force_simt = false;                            // SCD_DEBUG_FORCE_SIMT=1 (debug only)
   // tcgen05 path: plan-owned TMA descriptors of the B operands in device memory
-  // ([0,nseg) encoders, [nseg,2nseg) decoders, then 3 per PATCH layer) and fp16 RoPE tables
+  // ([0,nseg) encoders, [nseg,2nseg) decoders, then 3 per PATCH layer)
   void* tc_bmaps = nullptr;
-  void* rope_prod_h = nullptr;
-  void* rope_cons_h = nullptr;
 };
 
 namespace scd {

@@ -21,6 +21,7 @@
 #include <cuda_fp16.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstring>
 
 #include "ptx.cuh"
@@ -45,9 +46,9 @@ struct TcSeg {
 struct TcParams {
   CUtensorMap a_maps[TC_MAX_AMAPS];
   TcSeg segs[TC_MAX_SEGS];
+  uint32_t rope_g[64];                // theta^(-2j/d_h) / (2 pi) as a Q0.32 fraction of a turn
   const CUtensorMap* b_maps;          // plan-owned, global memory
   BatchDev batch;
-  const __half2* rope_h;              // [max_position][head_dim/2] (cos, sin) fp16
   int32_t n_segs, M, N, K;
   int32_t m_tiles, n_tiles, num_kb, block_n;
   int32_t a_kb_per_head;              // >0: A is [T, H, d_h] head-strided, k-blocks per head
@@ -58,6 +59,8 @@ struct TcParams {
 
 constexpr int BLOCK_M = 128, BLOCK_K = 64, STAGES = 4, TMEM_COLS = 512;
 constexpr int A_STAGE_BYTES = BLOCK_M * BLOCK_K * 2;        // 16 KB
+constexpr int SUB_N = 128;                                  // epilogue sub-tile width (columns)
+constexpr int STG_WARP_BYTES = 32 * SUB_N * 2;              // per-warp staging: 32 rows x 256 B
 
 struct __align__(8) TcBarriers {
   uint64_t full[STAGES], empty[STAGES], ready[STAGES];
@@ -66,13 +69,49 @@ struct __align__(8) TcBarriers {
 };
 
 static size_t tc_smem_bytes(int block_n) {
-  return 1024 /*align slack*/ + (size_t)STAGES * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) + sizeof(TcBarriers);
+  return 1024 /*align slack*/ + (size_t)STAGES * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) + 4 * STG_WARP_BYTES +
+         sizeof(TcBarriers);
 }
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
   return *reinterpret_cast<uint32_t*>(&v);
 }
+
+// (cos, sin) of position * theta^(-2j/d_h).  The angle is tracked as a 32-bit fraction of a
+// turn: pos * g wraps modulo 2^32 exactly, so the reduced angle in [-pi, pi) has an absolute
+// error <= pos * 2 pi * 2^-33 + 2^-24 turn (2.4e-5 rad at 32k positions) before the MUFU
+// approximations (2^-21 abs).  No table, no memory traffic.
+__device__ __forceinline__ float2 rope_cs(int pos, uint32_t g) {
+  const float x = (float)(int32_t)((uint32_t)pos * g) * 1.4629180792671596e-9f;   // 2 pi / 2^32
+  return make_float2(__cosf(x), __sinf(x));
+}
+
+// per-warp staging tile: row pitch `pitch` bytes (>= 128), 16-byte chunks XOR-swizzled on the
+// low 3 bits of the row so that row-per-thread writes and row-per-half-warp reads are both
+// bank-conflict free
+__device__ __forceinline__ void stg_put(uint8_t* stg, int pitch, int row, int chunk, uint4 v) {
+  *reinterpret_cast<uint4*>(stg + row * pitch + (((chunk & ~7) | ((chunk ^ row) & 7)) << 4)) = v;
+}
+
+// Copy the warp's staged sub-tile (32 rows x row_bytes) to global: `lpr` = row_bytes / 16 lanes
+// cover one row with one fully coalesced 16-B store each; row base pointers come from the
+// owning lane by shuffle (null = row beyond M).  `valid_bytes` masks the N tail.
+__device__ __forceinline__ void stg_copy_out(const uint8_t* stg, int pitch, int row_bytes, int valid_bytes,
+                                             unsigned long long my_row_ptr, unsigned long long byte_off, int lane) {
+  const int lpr = row_bytes >> 4;
+  const int rpi = 32 / lpr;
+  const int chunk = lane % lpr;
+  for (int it = 0; it < lpr; ++it) {
+    const int r = it * rpi + lane / lpr;
+    const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
+    const uint4 v = *reinterpret_cast<const uint4*>(stg + r * pitch + (((chunk & ~7) | ((chunk ^ r) & 7)) << 4));
+    if (base != 0ull && chunk * 16 < valid_bytes)
+      *reinterpret_cast<uint4*>(base + byte_off + (unsigned long long)chunk * 16) = v;
+  }
+}
+
+__device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
 // ---------------------------------------------------------------------------------
 // the kernel
@@ -86,7 +125,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   const uint32_t b_stage_bytes = (uint32_t)block_n * BLOCK_K * 2;
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
-  TcBarriers* bars = (TcBarriers*)(smem_b + STAGES * b_stage_bytes);
+  uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
+  TcBarriers* bars = (TcBarriers*)(smem_stg + 4 * STG_WARP_BYTES);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.n_segs * P.n_tiles * P.m_tiles;
@@ -166,8 +206,12 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     }
   } else if (warp >= 4 && warp < 8) {
     // ============================== epilogue ==============================
+    // One token row per thread (TMEM lane).  The tile is processed in sub-tiles of <= 128
+    // columns: TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced stores.
     const int ew = warp - 4;
     const int half = P.head_dim / 2;
+    uint8_t* stg = smem_stg + ew * STG_WARP_BYTES;
+    const int out_eb = (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2;
     int it = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
       const int m_tile = tile % P.m_tiles;
@@ -180,12 +224,20 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       const int n0 = n_tile * block_n;
       const int n_end = min(block_n, P.N - n0);              // valid columns in this tile
 
-      // per-row quantities (global loads issued before waiting for the accumulator)
+      // ---- per-row quantities (issued before waiting for the accumulator) ----
       int pos = 0;
-      long long slot = 0;
       float rs = 1.0f;
+      unsigned long long row_ptr = 0ull;                      // global address of this row's first tile column
       if (valid) {
-        if (EPI == EPI_KV) row_to_pos_slot(P.batch, row, pos, slot);
+        if (EPI == EPI_KV) {
+          long long slot;
+          row_to_pos_slot(P.batch, row, pos, slot);
+          const bool to1 = n0 >= P.split;
+          row_ptr = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
+                    ((unsigned long long)slot * P.pool_width + (to1 ? n0 - P.split : n0)) * 2ull;
+        } else {
+          row_ptr = (unsigned long long)sg.out0 + ((unsigned long long)row * P.N + n0) * (unsigned long long)out_eb;
+        }
         if ((EPI == EPI_KV || EPI == EPI_ACT) && sg.a_scale) rs = __ldg(sg.a_scale + row);
         if (EPI == EPI_KV && sg.rowscale_in) {
           float ss = 0.0f;
@@ -193,175 +245,142 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           rs *= rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
         }
       }
+      const float* cv = sg.col_vec ? sg.col_vec + n0 : nullptr;
 
       ptx::mbar_wait(&bars->tmem_full[acc], acc_phase);
       ptx::tc_fence_after();
       const uint32_t t_row = tmem_base + (uint32_t)(acc * block_n) + ((uint32_t)(ew * 32) << 16);
 
-      if (EPI == EPI_KV) {
-        const bool to1 = n0 >= P.split;
-        __nv_bfloat16* out = (__nv_bfloat16*)(to1 ? sg.out1 : sg.out0) + (size_t)slot * P.pool_width +
-                             (to1 ? n0 - P.split : n0);
-        int c = 0;
-        while (c < n_end) {
-          const int col = n0 + c;
-          if (col < sg.rope_cols && P.rope_style == SCD_ROPE_HALF) {
-            // one head: pairs (j, j + half), 16 pairs at a time
-            for (int j0 = 0; j0 < half; j0 += 16) {
-              uint32_t ra[16], rb[16];
-              ptx::tmem_ld16(t_row + c + j0, ra);
-              ptx::tmem_ld16(t_row + c + half + j0, rb);
-              ptx::tmem_ld_wait();
-              if (valid) {
-                const uint4* tp = reinterpret_cast<const uint4*>(P.rope_h + (size_t)pos * half + j0);
-                uint32_t oa[8], ob[8];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                  const uint4 cs4 = __ldg(tp + q);
-                  const uint32_t csw[4] = {cs4.x, cs4.y, cs4.z, cs4.w};
-                  float va[4], vb[4];
-#pragma unroll
-                  for (int e = 0; e < 4; ++e) {
-                    const int i = q * 4 + e;
-                    const float2 cs = __half22float2(*reinterpret_cast<const __half2*>(&csw[e]));
-                    float a = __uint_as_float(ra[i]) * rs, b = __uint_as_float(rb[i]) * rs;
-                    if (sg.col_vec) {
-                      a += __ldg(sg.col_vec + col + j0 + i);
-                      b += __ldg(sg.col_vec + col + half + j0 + i);
-                    }
-                    va[e] = a * cs.x - b * cs.y;
-                    vb[e] = b * cs.x + a * cs.y;
-                  }
-                  oa[q * 2] = pack_bf16x2(va[0], va[1]); oa[q * 2 + 1] = pack_bf16x2(va[2], va[3]);
-                  ob[q * 2] = pack_bf16x2(vb[0], vb[1]); ob[q * 2 + 1] = pack_bf16x2(vb[2], vb[3]);
-                }
-                uint4* da = reinterpret_cast<uint4*>(out + c + j0);
-                uint4* db = reinterpret_cast<uint4*>(out + c + half + j0);
-                da[0] = make_uint4(oa[0], oa[1], oa[2], oa[3]); da[1] = make_uint4(oa[4], oa[5], oa[6], oa[7]);
-                db[0] = make_uint4(ob[0], ob[1], ob[2], ob[3]); db[1] = make_uint4(ob[4], ob[5], ob[6], ob[7]);
-              }
-            }
-            c += P.head_dim;
-          } else {
-            // 32 columns: plain, or INTERLEAVED RoPE (pairs (2i, 2i+1) are adjacent)
-            uint32_t r[32];
-            ptx::tmem_ld32(t_row + c, r);
-            ptx::tmem_ld_wait();
-            if (valid) {
-              float v[32];
-#pragma unroll
-              for (int i = 0; i < 32; ++i) {
-                v[i] = __uint_as_float(r[i]) * rs;
-                if (sg.col_vec) v[i] += __ldg(sg.col_vec + col + i);
-              }
-              if (col < sg.rope_cols) {
-                const __half2* tp = P.rope_h + (size_t)pos * half + (col % P.head_dim) / 2;
-#pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                  const float2 cs = __half22float2(__ldg(tp + i));
-                  const float a = v[2 * i], b = v[2 * i + 1];
-                  v[2 * i] = a * cs.x - b * cs.y;
-                  v[2 * i + 1] = b * cs.x + a * cs.y;
-                }
-              }
-              uint4* dst = reinterpret_cast<uint4*>(out + c);
-#pragma unroll
-              for (int q = 0; q < 4; ++q)
-                dst[q] = make_uint4(pack_bf16x2(v[q * 8], v[q * 8 + 1]), pack_bf16x2(v[q * 8 + 2], v[q * 8 + 3]),
-                                    pack_bf16x2(v[q * 8 + 4], v[q * 8 + 5]), pack_bf16x2(v[q * 8 + 6], v[q * 8 + 7]));
-            }
-            c += 32;
-          }
-        }
-      } else if (EPI == EPI_CODES) {
-        // z = acc - c[n]; bf16 codes, or e4m3 with a per-row fp32 scale (tile spans all of N)
+      // e4m3 codes: the row scale needs the amax over all of N first (tile spans N)
+      float e4_scale = 1.0f;
+      if (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) {
         float amax = 0.0f;
-        if (P.code_dtype == SCD_E4M3_ROWSCALE) {
-          for (int c = 0; c < n_end; c += 32) {
-            uint32_t r[32];
-            ptx::tmem_ld32(t_row + c, r);
-            ptx::tmem_ld_wait();
-#pragma unroll
-            for (int i = 0; i < 32; ++i)
-              if (c + i < n_end) amax = fmaxf(amax, fabsf(__uint_as_float(r[i]) - __ldg(sg.col_vec + n0 + c + i)));
-          }
-        }
-        const float sc = amax > 0.0f ? amax / 448.0f : 1.0f;
-        if (P.code_dtype == SCD_E4M3_ROWSCALE && valid) sg.aux[row] = sc;
         for (int c = 0; c < n_end; c += 32) {
           uint32_t r[32];
           ptx::tmem_ld32(t_row + c, r);
           ptx::tmem_ld_wait();
-          if (valid) {
+#pragma unroll
+          for (int q = 0; q < 8; ++q) {
+            const float4 m4 = ldg_f4(cv + c + q * 4);
+            const float mm[4] = {m4.x, m4.y, m4.z, m4.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              if (c + q * 4 + e < n_end) amax = fmaxf(amax, fabsf(__uint_as_float(r[q * 4 + e]) - mm[e]));
+          }
+        }
+        e4_scale = amax > 0.0f ? amax / 448.0f : 1.0f;
+        if (valid) sg.aux[row] = e4_scale;
+      }
+      float ss_u = 0.0f;
+
+      for (int c0 = 0; c0 < n_end; c0 += SUB_N) {
+        const int sub_cols = min(SUB_N, block_n - c0);
+        const int row_bytes = sub_cols * out_eb;
+        const int pitch = row_bytes < 128 ? 128 : row_bytes;
+        const bool last_sub = c0 + SUB_N >= n_end;
+
+        if (EPI == EPI_KV && (n0 + c0) < sg.rope_cols && P.rope_style == SCD_ROPE_HALF) {
+          // ---- RoPE, HALF pairing: heads of this sub-tile, 16 pairs at a time ----
+          for (int hc = 0; hc < sub_cols; hc += P.head_dim)
+            for (int j0 = 0; j0 < half; j0 += 16) {
+              uint32_t ra[16], rb[16];
+              ptx::tmem_ld16(t_row + c0 + hc + j0, ra);
+              ptx::tmem_ld16(t_row + c0 + hc + half + j0, rb);
+              ptx::tmem_ld_wait();
+              uint32_t oa[8], ob[8];
+#pragma unroll
+              for (int q = 0; q < 4; ++q) {
+                float4 ma = make_float4(0.f, 0.f, 0.f, 0.f), mb = ma;
+                if (cv) { ma = ldg_f4(cv + c0 + hc + j0 + q * 4); mb = ldg_f4(cv + c0 + hc + half + j0 + q * 4); }
+                const float am[4] = {ma.x, ma.y, ma.z, ma.w}, bm[4] = {mb.x, mb.y, mb.z, mb.w};
+                float va[4], vb[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                  const int i = q * 4 + e;
+                  const float2 cs = rope_cs(pos, P.rope_g[j0 + i]);
+                  const float a = fmaf(__uint_as_float(ra[i]), rs, am[e]);
+                  const float b = fmaf(__uint_as_float(rb[i]), rs, bm[e]);
+                  va[e] = a * cs.x - b * cs.y;
+                  vb[e] = b * cs.x + a * cs.y;
+                }
+                oa[q * 2] = pack_bf16x2(va[0], va[1]); oa[q * 2 + 1] = pack_bf16x2(va[2], va[3]);
+                ob[q * 2] = pack_bf16x2(vb[0], vb[1]); ob[q * 2 + 1] = pack_bf16x2(vb[2], vb[3]);
+              }
+              const int ca = (hc + j0) >> 3, cb = (hc + half + j0) >> 3;
+              stg_put(stg, pitch, lane, ca, make_uint4(oa[0], oa[1], oa[2], oa[3]));
+              stg_put(stg, pitch, lane, ca + 1, make_uint4(oa[4], oa[5], oa[6], oa[7]));
+              stg_put(stg, pitch, lane, cb, make_uint4(ob[0], ob[1], ob[2], ob[3]));
+              stg_put(stg, pitch, lane, cb + 1, make_uint4(ob[4], ob[5], ob[6], ob[7]));
+            }
+        } else {
+          // ---- 32 columns at a time: plain epilogues, or INTERLEAVED RoPE (adjacent pairs) ----
+          for (int c = c0; c < c0 + sub_cols; c += 32) {
+            uint32_t r[32];
+            ptx::tmem_ld32(t_row + c, r);
+            ptx::tmem_ld_wait();
             float v[32];
 #pragma unroll
-            for (int i = 0; i < 32; ++i)
-              v[i] = (c + i < n_end) ? __uint_as_float(r[i]) - __ldg(sg.col_vec + n0 + c + i) : 0.0f;
-            if (P.code_dtype == SCD_E4M3_ROWSCALE) {
-              uint8_t* dst = (uint8_t*)sg.out0 + (size_t)row * P.N + n0 + c;
+            for (int q = 0; q < 8; ++q) {
+              float4 m4 = make_float4(0.f, 0.f, 0.f, 0.f);
+              if (cv) m4 = ldg_f4(cv + c + q * 4);
+              const float mm[4] = {m4.x, m4.y, m4.z, m4.w};
+#pragma unroll
+              for (int e = 0; e < 4; ++e) {
+                const int i = q * 4 + e;
+                float x = __uint_as_float(r[i]);
+                if (EPI == EPI_CODES) x -= mm[e];
+                else x = fmaf(x, rs, mm[e]);
+                if (EPI == EPI_ACT && P.act == SCD_ACT_SILU) x = __fdividef(x, 1.0f + __expf(-x));
+                if (c + i >= n_end) x = 0.0f;
+                if (EPI == EPI_U) ss_u = fmaf(x, x, ss_u);
+                v[i] = x;
+              }
+            }
+            if (EPI == EPI_KV && (n0 + c) < sg.rope_cols) {
+              const int f0 = ((n0 + c) % P.head_dim) >> 1;
+#pragma unroll
+              for (int i = 0; i < 16; ++i) {
+                const float2 cs = rope_cs(pos, P.rope_g[f0 + i]);
+                const float a = v[2 * i], b = v[2 * i + 1];
+                v[2 * i] = a * cs.x - b * cs.y;
+                v[2 * i + 1] = b * cs.x + a * cs.y;
+              }
+            }
+            if (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) {
 #pragma unroll
               for (int q = 0; q < 2; ++q) {
-                if (c + q * 16 >= n_end) break;
                 uint32_t w[4];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                   uint32_t b = 0;
 #pragma unroll
                   for (int y = 0; y < 4; ++y)
-                    b |= (uint32_t)float_to_e4m3_sat(__fdiv_rn(v[q * 16 + e * 4 + y], sc)) << (8 * y);
+                    b |= (uint32_t)float_to_e4m3_sat(__fdiv_rn(v[q * 16 + e * 4 + y], e4_scale)) << (8 * y);
                   w[e] = b;
                 }
-                reinterpret_cast<uint4*>(dst)[q] = make_uint4(w[0], w[1], w[2], w[3]);
+                stg_put(stg, pitch, lane, ((c - c0) >> 4) + q, make_uint4(w[0], w[1], w[2], w[3]));
               }
             } else {
-              __nv_bfloat16* dst = (__nv_bfloat16*)sg.out0 + (size_t)row * P.N + n0 + c;
 #pragma unroll
-              for (int q = 0; q < 4; ++q) {
-                if (c + q * 8 >= n_end) break;
-                reinterpret_cast<uint4*>(dst)[q] =
-                    make_uint4(pack_bf16x2(v[q * 8], v[q * 8 + 1]), pack_bf16x2(v[q * 8 + 2], v[q * 8 + 3]),
-                               pack_bf16x2(v[q * 8 + 4], v[q * 8 + 5]), pack_bf16x2(v[q * 8 + 6], v[q * 8 + 7]));
-              }
+              for (int q = 0; q < 4; ++q)
+                stg_put(stg, pitch, lane, ((c - c0) >> 3) + q,
+                        make_uint4(pack_bf16x2(v[q * 8], v[q * 8 + 1]), pack_bf16x2(v[q * 8 + 2], v[q * 8 + 3]),
+                                   pack_bf16x2(v[q * 8 + 4], v[q * 8 + 5]), pack_bf16x2(v[q * 8 + 6], v[q * 8 + 7])));
             }
           }
         }
-      } else {
-        // EPI_ACT: act(acc * rs + b1) ; EPI_U: acc + b2 and the row's partial sum of squares
-        float ss = 0.0f;
-        __nv_bfloat16* dst_row = (__nv_bfloat16*)sg.out0 + (size_t)row * P.N + n0;
-        for (int c = 0; c < n_end; c += 32) {
-          uint32_t r[32];
-          ptx::tmem_ld32(t_row + c, r);
-          ptx::tmem_ld_wait();
-          if (valid) {
-            float v[32];
-#pragma unroll
-            for (int i = 0; i < 32; ++i) {
-              float x = 0.0f;
-              if (c + i < n_end) {
-                x = __uint_as_float(r[i]) * rs;
-                if (sg.col_vec) x += __ldg(sg.col_vec + n0 + c + i);
-                if (EPI == EPI_ACT && P.act == SCD_ACT_SILU) x = x / (1.0f + __expf(-x));
-                if (EPI == EPI_U) ss += x * x;
-              }
-              v[i] = x;
-            }
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              if (c + q * 8 >= n_end) break;
-              reinterpret_cast<uint4*>(dst_row + c)[q] =
-                  make_uint4(pack_bf16x2(v[q * 8], v[q * 8 + 1]), pack_bf16x2(v[q * 8 + 2], v[q * 8 + 3]),
-                             pack_bf16x2(v[q * 8 + 4], v[q * 8 + 5]), pack_bf16x2(v[q * 8 + 6], v[q * 8 + 7]));
-            }
-          }
+        if (last_sub) {
+          // all TMEM reads of this tile are done: hand the accumulator back before the copy-out
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+        } else {
+          __syncwarp();
         }
-        if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)n_tile * P.M + row] = ss;
+        stg_copy_out(stg, pitch, row_bytes, (n_end - c0) * out_eb, row_ptr, (unsigned long long)c0 * out_eb, lane);
+        __syncwarp();
       }
-
-      // hand the accumulator buffer back to the MMA warp
-      ptx::tc_fence_before();
-      __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+      if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)n_tile * P.M + row] = ss_u;
     }
   } else if (AMODE == A_DEROPE && warp >= 8) {
     // ============================== A transform: deRoPE in shared memory ==============================
@@ -369,6 +388,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     // position c ^ (row & 7) (128-byte swizzle).  Channel pairs (j, j + d_h/2) of a head:
     //   d_h = 128: same chunk / element of two consecutive k-blocks (stages s, s+1)
     //   d_h =  64: chunks c and c + 4 of one k-block;  d_h = 32: chunks c and c + 2 (two heads per block)
+    // (cos, sin) of the row's position are computed once per tile and kept in registers.
     const int tr = threadIdx.x - 256;                 // 0..127 = row in tile
     const int half = P.head_dim / 2;
     int stage = 0;
@@ -379,35 +399,35 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       int pos = 0;
       long long slot;
       if (row < P.M) row_to_pos_slot(P.batch, row, pos, slot);
-      const __half2* trow = P.rope_h + (size_t)pos * half;
+      float2 cs[64];
+#pragma unroll
+      for (int j = 0; j < 64; ++j) cs[j] = (j < half) ? rope_cs(pos, P.rope_g[j]) : make_float2(1.f, 0.f);
       const uint32_t row_off = (uint32_t)(tr >> 3) * 1024 + (uint32_t)(tr & 7) * 128;
       const int step = P.head_dim == 128 ? 2 : 1;     // k-blocks consumed per iteration
+      const int pair_chunks = P.head_dim == 128 ? 8 : half / 8;         // chunks in the "a" half
+      const int groups = P.head_dim == 128 ? 1 : BLOCK_K / P.head_dim;  // heads per k-block
       for (int kb = 0; kb < P.num_kb; kb += step) {
         const int s0 = stage, s1 = (stage + 1) % STAGES;
         ptx::mbar_wait(&bars->full[s0], phase);
         if (step == 2) ptx::mbar_wait(&bars->full[s1], (s1 == 0) ? (phase ^ 1) : phase);
         uint8_t* ra = smem_a + s0 * A_STAGE_BYTES + row_off;
         uint8_t* rb = step == 2 ? smem_a + s1 * A_STAGE_BYTES + row_off : ra;
-        const int pair_chunks = P.head_dim == 128 ? 8 : half / 8;      // chunks in the "a" half
-        const int groups = P.head_dim == 128 ? 1 : BLOCK_K / P.head_dim; // heads per k-block
         for (int gidx = 0; gidx < groups; ++gidx)
-          for (int cc = 0; cc < pair_chunks; ++cc) {
+#pragma unroll
+          for (int cc = 0; cc < 8; ++cc) {
+            if (cc >= pair_chunks) break;
             const int ca = P.head_dim == 128 ? cc : gidx * (P.head_dim / 8) + cc;
             const int cb = P.head_dim == 128 ? cc : ca + pair_chunks;
             uint4* pa = reinterpret_cast<uint4*>(ra + ((ca ^ (tr & 7)) << 4));
             uint4* pb = reinterpret_cast<uint4*>(rb + ((cb ^ (tr & 7)) << 4));
             uint4 xa = *pa, xb = *pb;
-            const uint4 cs4a = __ldg(reinterpret_cast<const uint4*>(trow + cc * 8));
-            const uint4 cs4b = __ldg(reinterpret_cast<const uint4*>(trow + cc * 8 + 4));
-            const uint32_t csw[8] = {cs4a.x, cs4a.y, cs4a.z, cs4a.w, cs4b.x, cs4b.y, cs4b.z, cs4b.w};
             uint32_t* wa = reinterpret_cast<uint32_t*>(&xa);
             uint32_t* wb = reinterpret_cast<uint32_t*>(&xb);
 #pragma unroll
             for (int w = 0; w < 4; ++w) {
               const float2 a2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wa[w]));
               const float2 b2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wb[w]));
-              const float2 c0 = __half22float2(*reinterpret_cast<const __half2*>(&csw[2 * w]));
-              const float2 c1 = __half22float2(*reinterpret_cast<const __half2*>(&csw[2 * w + 1]));
+              const float2 c0 = cs[cc * 8 + 2 * w], c1 = cs[cc * 8 + 2 * w + 1];
               // rotation by -phi:  a' = a cos + b sin ; b' = b cos - a sin
               wa[w] = pack_bf16x2(a2.x * c0.x + b2.x * c0.y, a2.y * c1.x + b2.y * c1.y);
               wb[w] = pack_bf16x2(b2.x * c0.x - a2.x * c0.y, b2.y * c1.x - a2.y * c1.y);
@@ -493,12 +513,6 @@ static int pick_block_n_cover(int n) {          // smallest multiple of 16 cover
   return b > 256 ? 256 : b;
 }
 
-// fp16 (cos, sin) tables, built from the plan's fp32 tables
-__global__ void rope_to_half_kernel(const float2* __restrict__ src, __half2* __restrict__ dst, size_t n) {
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
-    dst[i] = __floats2half2_rn(src[i].x, src[i].y);
-}
-
 scd_status_t tc_supported(const scd_plan_t* p, const scd_layer_desc_t* layers) {
   const scd_model_desc_t& m = p->model;
   if (p->D % 32) return fail(SCD_E_UNSUPPORTED, "D = %d not a multiple of 32", p->D);
@@ -541,22 +555,7 @@ scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
     return fail(SCD_E_CUDA, "cudaMemcpy(tensor maps)");
   p->tc_bmaps = d;
 
-  const size_t n = (size_t)m.max_position * (m.head_dim / 2);
-  void* hc = nullptr;
-  if (cudaMalloc(&hc, n * sizeof(__half2)) != cudaSuccess) return fail(SCD_E_NOMEM, "cudaMalloc(rope fp16)");
-  p->allocs.push_back(hc);
-  rope_to_half_kernel<<<1024, 256, 0, s>>>(p->rope_cons, (__half2*)hc, n);
-  p->rope_cons_h = hc;
-  if (p->rope_prod == p->rope_cons) {
-    p->rope_prod_h = hc;
-  } else {
-    void* hp = nullptr;
-    if (cudaMalloc(&hp, n * sizeof(__half2)) != cudaSuccess) return fail(SCD_E_NOMEM, "cudaMalloc(rope fp16)");
-    p->allocs.push_back(hp);
-    rope_to_half_kernel<<<1024, 256, 0, s>>>(p->rope_prod, (__half2*)hp, n);
-    p->rope_prod_h = hp;
-  }
-  if (cudaGetLastError() != cudaSuccess) return fail(SCD_E_CUDA, "rope_to_half_kernel launch failed");
+  (void)s;
   return SCD_OK;
 }
 
@@ -597,7 +596,15 @@ static void fill_common(const scd_plan_t* p, const scd_batch_t* b, bool pages, b
   P.batch.total_tokens = b->total_tokens;
   P.batch.max_pages_per_seq = b->max_pages_per_seq;
   P.batch.block_size = p->model.block_size;
-  P.rope_h = (const __half2*)(producer ? p->rope_prod_h : p->rope_cons_h);
+  {
+    // frequencies as Q0.32 fractions of a turn, from fp64 (exact modular angle arithmetic in the kernel)
+    const double theta = producer ? p->model.rope_theta_producer : p->model.rope_theta_consumer;
+    for (int j = 0; j < p->model.head_dim / 2 && j < 64; ++j) {
+      double turns = pow(theta, -2.0 * j / p->model.head_dim) / 6.283185307179586476925286766559;
+      turns -= floor(turns);
+      P.rope_g[j] = (uint32_t)llround(turns * 4294967296.0);
+    }
+  }
   P.head_dim = p->model.head_dim;
   P.rope_style = p->model.rope_style;
   P.act = p->model.patch_act;
