@@ -142,7 +142,7 @@ static size_t patch_workspace(const scd_plan_t* p, int32_t T) {
   for (auto& pp : p->patches) d_a = pp.d_a > d_a ? pp.d_a : d_a;
   const int d = p->model.d_model;
   return align_up((size_t)T * d_a * es, 128) + align_up((size_t)T * d * es, 128) +
-         align_up((size_t)((d + 127) / 128) * T * 4, 128);
+         align_up((size_t)(2 * ((d + 127) / 128)) * T * 4, 128);   // sum-of-squares partials
 }
 
 // ---------------------------------------------------------------------------------

@@ -50,27 +50,36 @@ struct TcParams {
   const CUtensorMap* b_maps;          // plan-owned, global memory
   BatchDev batch;
   int32_t n_segs, M, N, K;
-  int32_t m_tiles, n_tiles, num_kb, block_n;
+  int32_t m_tiles, n_tiles, num_kb, block_n, stages;
   int32_t a_kb_per_head;              // >0: A is [T, H, d_h] head-strided, k-blocks per head
   int32_t split, pool_width, head_dim, rope_style, act, code_dtype;
   int32_t n_partials, rms_dim;
   float rms_eps;
 };
 
-constexpr int BLOCK_M = 128, BLOCK_K = 64, STAGES = 4, TMEM_COLS = 512;
+constexpr int BLOCK_M = 128, BLOCK_K = 64, MAX_STAGES = 8, TMEM_COLS = 512;
+constexpr int EPI_WARPS = 8;                                // two per TMEM lane quadrant, splitting the columns
 constexpr int A_STAGE_BYTES = BLOCK_M * BLOCK_K * 2;        // 16 KB
 constexpr int SUB_N = 128;                                  // epilogue sub-tile width (columns)
 constexpr int STG_WARP_BYTES = 32 * SUB_N * 2;              // per-warp staging: 32 rows x 256 B
 
 struct __align__(8) TcBarriers {
-  uint64_t full[STAGES], empty[STAGES], ready[STAGES];
+  uint64_t full[MAX_STAGES], empty[MAX_STAGES], ready[MAX_STAGES];
   uint64_t tmem_full[2], tmem_empty[2];
   uint32_t tmem_base;
 };
 
-static size_t tc_smem_bytes(int block_n) {
-  return 1024 /*align slack*/ + (size_t)STAGES * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) + 4 * STG_WARP_BYTES +
-         sizeof(TcBarriers);
+static size_t tc_smem_bytes(int block_n, int stages) {
+  return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) +
+         EPI_WARPS * STG_WARP_BYTES + sizeof(TcBarriers);
+}
+static int tc_pick_stages(int block_n, int num_kb, bool even) {
+  const size_t budget = 232448 - 1024 - EPI_WARPS * STG_WARP_BYTES - sizeof(TcBarriers);
+  int st = (int)(budget / (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2));
+  st = st > MAX_STAGES ? MAX_STAGES : st;
+  if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty
+  if (even && (st & 1)) --st;                                                  // deRoPE pairs k-blocks: keep it even
+  return st < 2 ? 2 : st;
 }
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
@@ -97,17 +106,31 @@ __device__ __forceinline__ void stg_put(uint8_t* stg, int pitch, int row, int ch
 // Copy the warp's staged sub-tile (32 rows x row_bytes) to global: `lpr` = row_bytes / 16 lanes
 // cover one row with one fully coalesced 16-B store each; row base pointers come from the
 // owning lane by shuffle (null = row beyond M).  `valid_bytes` masks the N tail.
-__device__ __forceinline__ void stg_copy_out(const uint8_t* stg, int pitch, int row_bytes, int valid_bytes,
-                                             unsigned long long my_row_ptr, unsigned long long byte_off, int lane) {
-  const int lpr = row_bytes >> 4;
-  const int rpi = 32 / lpr;
+template <int LPR>
+__device__ __forceinline__ void stg_copy_out_t(const uint8_t* stg, int pitch, int valid_bytes,
+                                               unsigned long long my_row_ptr, unsigned long long byte_off, int lane) {
+  constexpr int lpr = LPR;
+  constexpr int rpi = 32 / lpr;
   const int chunk = lane % lpr;
+#pragma unroll
   for (int it = 0; it < lpr; ++it) {
     const int r = it * rpi + lane / lpr;
     const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
     const uint4 v = *reinterpret_cast<const uint4*>(stg + r * pitch + (((chunk & ~7) | ((chunk ^ r) & 7)) << 4));
     if (base != 0ull && chunk * 16 < valid_bytes)
       *reinterpret_cast<uint4*>(base + byte_off + (unsigned long long)chunk * 16) = v;
+  }
+}
+__device__ __forceinline__ void stg_copy_out(const uint8_t* stg, int pitch, int row_bytes, int valid_bytes,
+                                             unsigned long long my_row_ptr, unsigned long long byte_off, int lane) {
+  int lpr = 1;
+  while (lpr * 16 < row_bytes) lpr <<= 1;             // lanes per row: next power of two
+  switch (lpr) {
+    case 16: stg_copy_out_t<16>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
+    case 8: stg_copy_out_t<8>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
+    case 4: stg_copy_out_t<4>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
+    case 2: stg_copy_out_t<2>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
+    default: stg_copy_out_t<1>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
   }
 }
 
@@ -117,16 +140,17 @@ __device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterp
 // the kernel
 // ---------------------------------------------------------------------------------
 template <int EPI, int AMODE>
-__global__ void __launch_bounds__(AMODE == A_DEROPE ? 384 : 256, 1)
+__global__ void __launch_bounds__(AMODE == A_DEROPE ? 512 : 384, 1)
 tc_gemm_kernel(const __grid_constant__ TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int block_n = P.block_n;
   const uint32_t b_stage_bytes = (uint32_t)block_n * BLOCK_K * 2;
+  const int STAGES = P.stages;
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
   uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
-  TcBarriers* bars = (TcBarriers*)(smem_stg + 4 * STG_WARP_BYTES);
+  TcBarriers* bars = (TcBarriers*)(smem_stg + EPI_WARPS * STG_WARP_BYTES);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.n_segs * P.n_tiles * P.m_tiles;
@@ -139,7 +163,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
-      ptx::mbar_init(&bars->tmem_empty[a], 4);
+      ptx::mbar_init(&bars->tmem_empty[a], EPI_WARPS);
     }
     ptx::fence_barrier_init();
   }
@@ -204,13 +228,19 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         ptx::mma_commit(&bars->tmem_full[acc]);
       }
     }
-  } else if (warp >= 4 && warp < 8) {
+  } else if (warp >= 4 && warp < 4 + EPI_WARPS) {
     // ============================== epilogue ==============================
-    // One token row per thread (TMEM lane).  The tile is processed in sub-tiles of <= 128
-    // columns: TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced stores.
-    const int ew = warp - 4;
+    // One token row per thread (TMEM lane); warps w and w+4 share a lane quadrant and split the
+    // tile's columns into two groups.  Each group is processed in sub-tiles of <= 128 columns:
+    // TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced stores.
+    const int ew = (warp - 4) & 3;                    // TMEM lane quadrant (= warp % 4)
+    const int grp = (warp - 4) >> 2;                  // column group 0 / 1
     const int half = P.head_dim / 2;
-    uint8_t* stg = smem_stg + ew * STG_WARP_BYTES;
+    uint8_t* stg = smem_stg + (warp - 4) * STG_WARP_BYTES;
+    // split only when both halves keep whole heads (RoPE) and whole 32-column TMEM chunks
+    const int gran = (EPI == EPI_KV && P.head_dim > 32) ? P.head_dim : 32;
+    const bool split_cols = (block_n % (2 * gran)) == 0;
+    const int grp_cols = split_cols ? block_n / 2 : block_n;
     const int out_eb = (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2;
     int it = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
@@ -223,6 +253,9 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       const bool valid = row < P.M;
       const int n0 = n_tile * block_n;
       const int n_end = min(block_n, P.N - n0);              // valid columns in this tile
+      const int g_begin = grp * grp_cols;                     // this warp's columns [g_begin, g_end) of the tile
+      const int g_end = min(n_end, g_begin + grp_cols);
+      const bool has_work = (grp == 0 || split_cols) && g_begin < n_end;
 
       // ---- per-row quantities (issued before waiting for the accumulator) ----
       int pos = 0;
@@ -253,7 +286,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // e4m3 codes: the row scale needs the amax over all of N first (tile spans N)
       float e4_scale = 1.0f;
-      if (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) {
+      if (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE && has_work) {
         float amax = 0.0f;
         for (int c = 0; c < n_end; c += 32) {
           uint32_t r[32];
@@ -269,15 +302,22 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           }
         }
         e4_scale = amax > 0.0f ? amax / 448.0f : 1.0f;
-        if (valid) sg.aux[row] = e4_scale;
+        if (valid && grp == 0) sg.aux[row] = e4_scale;
       }
       float ss_u = 0.0f;
 
-      for (int c0 = 0; c0 < n_end; c0 += SUB_N) {
-        const int sub_cols = min(SUB_N, block_n - c0);
+      if (!has_work) {                                        // nothing to read: release the accumulator
+        if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = 0.0f;
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+        continue;
+      }
+      for (int c0 = g_begin; c0 < g_end; c0 += SUB_N) {
+        const int sub_cols = min(SUB_N, g_begin + grp_cols - c0);
         const int row_bytes = sub_cols * out_eb;
         const int pitch = row_bytes < 128 ? 128 : row_bytes;
-        const bool last_sub = c0 + SUB_N >= n_end;
+        const bool last_sub = c0 + SUB_N >= g_end;
 
         if (EPI == EPI_KV && (n0 + c0) < sg.rope_cols && P.rope_style == SCD_ROPE_HALF) {
           // ---- RoPE, HALF pairing: heads of this sub-tile, 16 pairs at a time ----
@@ -380,16 +420,16 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         stg_copy_out(stg, pitch, row_bytes, (n_end - c0) * out_eb, row_ptr, (unsigned long long)c0 * out_eb, lane);
         __syncwarp();
       }
-      if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)n_tile * P.M + row] = ss_u;
+      if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = ss_u;
     }
-  } else if (AMODE == A_DEROPE && warp >= 8) {
+  } else if (AMODE == A_DEROPE && warp >= 4 + EPI_WARPS) {
     // ============================== A transform: deRoPE in shared memory ==============================
     // One token row per thread.  A k-block row is 128 B = 8 chunks of 16 B, chunk c stored at
     // position c ^ (row & 7) (128-byte swizzle).  Channel pairs (j, j + d_h/2) of a head:
     //   d_h = 128: same chunk / element of two consecutive k-blocks (stages s, s+1)
     //   d_h =  64: chunks c and c + 4 of one k-block;  d_h = 32: chunks c and c + 2 (two heads per block)
     // (cos, sin) of the row's position are computed once per tile and kept in registers.
-    const int tr = threadIdx.x - 256;                 // 0..127 = row in tile
+    const int tr = threadIdx.x - (4 + EPI_WARPS) * 32;   // 0..127 = row in tile
     const int half = P.head_dim / 2;
     int stage = 0;
     uint32_t phase = 0;
@@ -399,9 +439,12 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       int pos = 0;
       long long slot;
       if (row < P.M) row_to_pos_slot(P.batch, row, pos, slot);
-      float2 cs[64];
+      __half2 cs[64];                                   // fp16 (2^-12 abs) is below the bf16 operand rounding
 #pragma unroll
-      for (int j = 0; j < 64; ++j) cs[j] = (j < half) ? rope_cs(pos, P.rope_g[j]) : make_float2(1.f, 0.f);
+      for (int j = 0; j < 64; ++j) {
+        const float2 f = (j < half) ? rope_cs(pos, P.rope_g[j]) : make_float2(1.f, 0.f);
+        cs[j] = __floats2half2_rn(f.x, f.y);
+      }
       const uint32_t row_off = (uint32_t)(tr >> 3) * 1024 + (uint32_t)(tr & 7) * 128;
       const int step = P.head_dim == 128 ? 2 : 1;     // k-blocks consumed per iteration
       const int pair_chunks = P.head_dim == 128 ? 8 : half / 8;         // chunks in the "a" half
@@ -427,7 +470,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
             for (int w = 0; w < 4; ++w) {
               const float2 a2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wa[w]));
               const float2 b2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wb[w]));
-              const float2 c0 = cs[cc * 8 + 2 * w], c1 = cs[cc * 8 + 2 * w + 1];
+              const float2 c0 = __half22float2(cs[cc * 8 + 2 * w]), c1 = __half22float2(cs[cc * 8 + 2 * w + 1]);
               // rotation by -phi:  a' = a cos + b sin ; b' = b cos - a sin
               wa[w] = pack_bf16x2(a2.x * c0.x + b2.x * c0.y, a2.y * c1.x + b2.y * c1.y);
               wb[w] = pack_bf16x2(b2.x * c0.x - a2.x * c0.y, b2.y * c1.x - a2.y * c1.y);
@@ -569,7 +612,8 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.num_kb = (P.K + BLOCK_K - 1) / BLOCK_K;
   const int total = P.n_segs * P.m_tiles * P.n_tiles;
   if (total <= 0) return SCD_OK;
-  const size_t smem = tc_smem_bytes(P.block_n);
+  P.stages = tc_pick_stages(P.block_n, P.num_kb, AMODE == A_DEROPE);
+  const size_t smem = tc_smem_bytes(P.block_n, P.stages);
   static thread_local size_t configured = 0;   // per instantiation
   if (configured < smem) {
     cudaError_t e = cudaFuncSetAttribute(tc_gemm_kernel<EPI, AMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -578,7 +622,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   }
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
-  tc_gemm_kernel<EPI, AMODE><<<grid, AMODE == A_DEROPE ? 384 : 256, smem, s>>>(P);
+  tc_gemm_kernel<EPI, AMODE><<<grid, AMODE == A_DEROPE ? 512 : 384, smem, s>>>(P);
   prof_end(s, 100 + 10 * EPI + AMODE);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));
@@ -775,7 +819,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     if ((st = make_map(&P.a_maps[0], ws_act, pp.d_a, T, 1, (uint64_t)pp.d_a * 2, (uint64_t)pp.d_a * 2 * T, BLOCK_M, 1)) != SCD_OK) return st;
     P.segs[0].col_vec = pp.b2; P.segs[0].out0 = ws_u; P.segs[0].aux = rms ? ws_ss : nullptr;
     P.segs[0].b_map = 2 * nseg + 3 * (int)j + 1;
-    const int n_partials = (d + P.block_n - 1) / P.block_n;
+    const int n_partials = 2 * ((d + P.block_n - 1) / P.block_n);   // two column groups per n-tile
     if ((st = launch_tc<EPI_U, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     // GEMM-3: [T, d] x [d, 2D]
     fill_common(p, batch, true, false, P);
