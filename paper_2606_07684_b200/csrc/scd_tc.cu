@@ -62,6 +62,7 @@ constexpr int EPI_WARPS = 8;                                // two per TMEM lane
 constexpr int A_STAGE_BYTES = BLOCK_M * BLOCK_K * 2;        // 16 KB
 constexpr int SUB_N = 128;                                  // epilogue sub-tile width (columns)
 constexpr int STG_WARP_BYTES = 32 * SUB_N * 2;              // per-warp staging: 32 rows x 256 B
+constexpr int VEC_WARP_BYTES = 256 * 4;                     // per-warp copy of the tile's mean / bias slice
 
 struct __align__(8) TcBarriers {
   uint64_t full[MAX_STAGES], empty[MAX_STAGES], ready[MAX_STAGES];
@@ -71,10 +72,10 @@ struct __align__(8) TcBarriers {
 
 static size_t tc_smem_bytes(int block_n, int stages) {
   return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) +
-         EPI_WARPS * STG_WARP_BYTES + sizeof(TcBarriers);
+         EPI_WARPS * (STG_WARP_BYTES + VEC_WARP_BYTES) + sizeof(TcBarriers);
 }
 static int tc_pick_stages(int block_n, int num_kb, bool even) {
-  const size_t budget = 232448 - 1024 - EPI_WARPS * STG_WARP_BYTES - sizeof(TcBarriers);
+  const size_t budget = 232448 - 1024 - EPI_WARPS * (STG_WARP_BYTES + VEC_WARP_BYTES) - sizeof(TcBarriers);
   int st = (int)(budget / (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2));
   st = st > MAX_STAGES ? MAX_STAGES : st;
   if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty
@@ -96,32 +97,33 @@ __device__ __forceinline__ float2 rope_cs(int pos, uint32_t g) {
   return make_float2(__cosf(x), __sinf(x));
 }
 
-// per-warp staging tile: row pitch `pitch` bytes (>= 128), 16-byte chunks XOR-swizzled on the
-// low 3 bits of the row so that row-per-thread writes and row-per-half-warp reads are both
-// bank-conflict free
-__device__ __forceinline__ void stg_put(uint8_t* stg, int pitch, int row, int chunk, uint4 v) {
-  *reinterpret_cast<uint4*>(stg + row * pitch + (((chunk & ~7) | ((chunk ^ row) & 7)) << 4)) = v;
+// per-warp staging tile (shared-space address `stg`): row pitch `pitch` bytes (>= 128), 16-byte
+// chunks XOR-swizzled on the low 3 bits of the row so that row-per-thread writes and
+// row-per-half-warp reads are both bank-conflict free
+__device__ __forceinline__ uint32_t stg_addr(uint32_t stg, int pitch, int row, int chunk) {
+  return stg + row * pitch + (((chunk & ~7) | ((chunk ^ row) & 7)) << 4);
+}
+__device__ __forceinline__ void stg_put(uint32_t stg, int pitch, int row, int chunk, uint4 v) {
+  ptx::sts128(stg_addr(stg, pitch, row, chunk), v);
 }
 
-// Copy the warp's staged sub-tile (32 rows x row_bytes) to global: `lpr` = row_bytes / 16 lanes
-// cover one row with one fully coalesced 16-B store each; row base pointers come from the
-// owning lane by shuffle (null = row beyond M).  `valid_bytes` masks the N tail.
+// Copy the warp's staged sub-tile (32 rows x row_bytes) to global: LPR lanes cover one row with
+// one fully coalesced 16-B store each; row base pointers come from the owning lane by shuffle
+// (null = row beyond M).  `valid_bytes` masks the N tail.
 template <int LPR>
-__device__ __forceinline__ void stg_copy_out_t(const uint8_t* stg, int pitch, int valid_bytes,
-                                               unsigned long long my_row_ptr, unsigned long long byte_off, int lane) {
-  constexpr int lpr = LPR;
-  constexpr int rpi = 32 / lpr;
-  const int chunk = lane % lpr;
+__device__ __forceinline__ void stg_copy_out_t(uint32_t stg, int pitch, int valid_bytes, unsigned long long my_row_ptr,
+                                               unsigned long long byte_off, int lane) {
+  constexpr int rpi = 32 / LPR;
+  const int chunk = lane % LPR;
 #pragma unroll
-  for (int it = 0; it < lpr; ++it) {
-    const int r = it * rpi + lane / lpr;
+  for (int it = 0; it < LPR; ++it) {
+    const int r = it * rpi + lane / LPR;
     const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
-    const uint4 v = *reinterpret_cast<const uint4*>(stg + r * pitch + (((chunk & ~7) | ((chunk ^ r) & 7)) << 4));
-    if (base != 0ull && chunk * 16 < valid_bytes)
-      *reinterpret_cast<uint4*>(base + byte_off + (unsigned long long)chunk * 16) = v;
+    const uint4 v = ptx::lds128(stg_addr(stg, pitch, r, chunk));
+    if (base != 0ull && chunk * 16 < valid_bytes) ptx::stg128(base + byte_off + (unsigned long long)chunk * 16, v);
   }
 }
-__device__ __forceinline__ void stg_copy_out(const uint8_t* stg, int pitch, int row_bytes, int valid_bytes,
+__device__ __forceinline__ void stg_copy_out(uint32_t stg, int pitch, int row_bytes, int valid_bytes,
                                              unsigned long long my_row_ptr, unsigned long long byte_off, int lane) {
   int lpr = 1;
   while (lpr * 16 < row_bytes) lpr <<= 1;             // lanes per row: next power of two
@@ -135,6 +137,64 @@ __device__ __forceinline__ void stg_copy_out(const uint8_t* stg, int pitch, int 
 }
 
 __device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+
+// RoPE epilogue of one K tile, specialised for HALF pairing, head_dim 128, 256-column tiles (two
+// heads).  The warp pair of a lane quadrant splits the FREQUENCIES, not the columns: warp JG owns
+// j in [32 JG, 32 JG + 32) of both heads, so every (cos, sin) is computed once and used twice.
+// Staged row = 4 runs of 32 columns: (head 0, a) (head 0, b) (head 1, a) (head 1, b).
+template <int JG>
+__device__ __forceinline__ void rope_tile_h128(const TcParams& P, uint32_t t_row, uint32_t stg, uint32_t wvec, int pos,
+                                               float rs, int lane) {
+#pragma unroll
+  for (int jj = 0; jj < 32; jj += 16) {
+    float2 cs[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) cs[i] = rope_cs(pos, P.rope_g[JG * 32 + jj + i]);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      uint32_t ra[16], rb[16];
+      const int ca = h * 128 + JG * 32 + jj;          // tile column of the "a" elements; "b" = +64
+      ptx::tmem_ld16(t_row + ca, ra);
+      ptx::tmem_ld16(t_row + ca + 64, rb);
+      ptx::tmem_ld_wait();
+      uint32_t oa[8], ob[8];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const float4 ma = ptx::lds_f4(wvec + (ca + q * 4) * 4), mb = ptx::lds_f4(wvec + (ca + 64 + q * 4) * 4);
+        const float am[4] = {ma.x, ma.y, ma.z, ma.w}, bm[4] = {mb.x, mb.y, mb.z, mb.w};
+        float va[4], vb[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          const int i = q * 4 + e;
+          const float a = fmaf(__uint_as_float(ra[i]), rs, am[e]);
+          const float b = fmaf(__uint_as_float(rb[i]), rs, bm[e]);
+          va[e] = a * cs[i].x - b * cs[i].y;
+          vb[e] = b * cs[i].x + a * cs[i].y;
+        }
+        oa[q * 2] = pack_bf16x2(va[0], va[1]); oa[q * 2 + 1] = pack_bf16x2(va[2], va[3]);
+        ob[q * 2] = pack_bf16x2(vb[0], vb[1]); ob[q * 2 + 1] = pack_bf16x2(vb[2], vb[3]);
+      }
+      const int k0 = h * 8 + (jj >> 3);               // chunk of run (h, a); run (h, b) = +4
+      stg_put(stg, 256, lane, k0, make_uint4(oa[0], oa[1], oa[2], oa[3]));
+      stg_put(stg, 256, lane, k0 + 1, make_uint4(oa[4], oa[5], oa[6], oa[7]));
+      stg_put(stg, 256, lane, k0 + 4, make_uint4(ob[0], ob[1], ob[2], ob[3]));
+      stg_put(stg, 256, lane, k0 + 5, make_uint4(ob[4], ob[5], ob[6], ob[7]));
+    }
+  }
+}
+// copy-out of the 4-run layout above: lane l of a half-warp holds run l / 4, chunk l % 4
+template <int JG>
+__device__ __forceinline__ void rope_tile_h128_copy_out(uint32_t stg, unsigned long long my_row_ptr, int lane) {
+  const int l = lane & 15;
+  const unsigned long long off = (unsigned long long)(((l >> 3) * 128 + ((l >> 2) & 1) * 64 + JG * 32 + (l & 3) * 8) * 2);
+#pragma unroll
+  for (int it = 0; it < 16; ++it) {
+    const int r = it * 2 + (lane >> 4);
+    const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
+    const uint4 v = ptx::lds128(stg_addr(stg, 256, r, l));
+    if (base != 0ull) ptx::stg128(base + off, v);
+  }
+}
 
 // ---------------------------------------------------------------------------------
 // the kernel
@@ -150,7 +210,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
   uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
-  TcBarriers* bars = (TcBarriers*)(smem_stg + EPI_WARPS * STG_WARP_BYTES);
+  uint8_t* smem_vec = smem_stg + EPI_WARPS * STG_WARP_BYTES;
+  TcBarriers* bars = (TcBarriers*)(smem_vec + EPI_WARPS * VEC_WARP_BYTES);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.n_segs * P.n_tiles * P.m_tiles;
@@ -188,7 +249,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
         for (int kb = 0; kb < P.num_kb; ++kb) {
-          ptx::mbar_wait(&bars->empty[stage], phase ^ 1);
+          ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
           ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES + b_stage_bytes);
           if (P.a_kb_per_head > 0)
             ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES, am, &bars->full[stage],
@@ -211,11 +272,11 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
-        ptx::mbar_wait(&bars->tmem_empty[acc], acc_phase ^ 1);
+        ptx::mbar_wait_suspend(&bars->tmem_empty[acc], acc_phase ^ 1);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(acc * block_n);
         for (int kb = 0; kb < P.num_kb; ++kb) {
-          ptx::mbar_wait(AMODE == A_DEROPE ? &bars->ready[stage] : &bars->full[stage], phase);
+          ptx::mbar_wait_suspend(AMODE == A_DEROPE ? &bars->ready[stage] : &bars->full[stage], phase);
           ptx::tc_fence_after();
           const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
           const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * b_stage_bytes));
@@ -236,7 +297,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     const int ew = (warp - 4) & 3;                    // TMEM lane quadrant (= warp % 4)
     const int grp = (warp - 4) >> 2;                  // column group 0 / 1
     const int half = P.head_dim / 2;
-    uint8_t* stg = smem_stg + (warp - 4) * STG_WARP_BYTES;
+    const uint32_t stg = ptx::smem_u32(smem_stg + (warp - 4) * STG_WARP_BYTES);
+    const uint32_t wvec = ptx::smem_u32(smem_vec + (warp - 4) * VEC_WARP_BYTES);
     // split only when both halves keep whole heads (RoPE) and whole 32-column TMEM chunks
     const int gran = (EPI == EPI_KV && P.head_dim > 32) ? P.head_dim : 32;
     const bool split_cols = (block_n % (2 * gran)) == 0;
@@ -278,9 +340,20 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           rs *= rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
         }
       }
-      const float* cv = sg.col_vec ? sg.col_vec + n0 : nullptr;
+      // this warp's copy of the tile's mean / bias slice (zeros when absent): wvec[c] for tile column c
+      {
+        float4 m0 = make_float4(0.f, 0.f, 0.f, 0.f), m1 = m0;
+        if (sg.col_vec) {
+          m0 = ldg_f4(sg.col_vec + n0 + lane * 4);
+          if (block_n > 128) m1 = ldg_f4(sg.col_vec + n0 + 128 + lane * 4);
+        }
+        __syncwarp();
+        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(m0.x), "f"(m0.y), "f"(m0.z), "f"(m0.w) : "memory");
+        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + 512 + lane * 16), "f"(m1.x), "f"(m1.y), "f"(m1.z), "f"(m1.w) : "memory");
+        __syncwarp();
+      }
 
-      ptx::mbar_wait(&bars->tmem_full[acc], acc_phase);
+      ptx::mbar_wait_suspend(&bars->tmem_full[acc], acc_phase);
       ptx::tc_fence_after();
       const uint32_t t_row = tmem_base + (uint32_t)(acc * block_n) + ((uint32_t)(ew * 32) << 16);
 
@@ -294,7 +367,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           ptx::tmem_ld_wait();
 #pragma unroll
           for (int q = 0; q < 8; ++q) {
-            const float4 m4 = ldg_f4(cv + c + q * 4);
+            const float4 m4 = ptx::lds_f4(wvec + (c + q * 4) * 4);
             const float mm[4] = {m4.x, m4.y, m4.z, m4.w};
 #pragma unroll
             for (int e = 0; e < 4; ++e)
@@ -306,6 +379,18 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       }
       float ss_u = 0.0f;
 
+      if (EPI == EPI_KV && n0 < sg.rope_cols && P.rope_style == SCD_ROPE_HALF && P.head_dim == 128 && block_n == 256 &&
+          n_end == 256) {
+        if (grp == 0) rope_tile_h128<0>(P, t_row, stg, wvec, pos, rs, lane);
+        else rope_tile_h128<1>(P, t_row, stg, wvec, pos, rs, lane);
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+        if (grp == 0) rope_tile_h128_copy_out<0>(stg, row_ptr, lane);
+        else rope_tile_h128_copy_out<1>(stg, row_ptr, lane);
+        __syncwarp();
+        continue;
+      }
       if (!has_work) {                                        // nothing to read: release the accumulator
         if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = 0.0f;
         ptx::tc_fence_before();
@@ -330,8 +415,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
               uint32_t oa[8], ob[8];
 #pragma unroll
               for (int q = 0; q < 4; ++q) {
-                float4 ma = make_float4(0.f, 0.f, 0.f, 0.f), mb = ma;
-                if (cv) { ma = ldg_f4(cv + c0 + hc + j0 + q * 4); mb = ldg_f4(cv + c0 + hc + half + j0 + q * 4); }
+                const float4 ma = ptx::lds_f4(wvec + (c0 + hc + j0 + q * 4) * 4);
+                const float4 mb = ptx::lds_f4(wvec + (c0 + hc + half + j0 + q * 4) * 4);
                 const float am[4] = {ma.x, ma.y, ma.z, ma.w}, bm[4] = {mb.x, mb.y, mb.z, mb.w};
                 float va[4], vb[4];
 #pragma unroll
@@ -361,8 +446,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
             float v[32];
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-              float4 m4 = make_float4(0.f, 0.f, 0.f, 0.f);
-              if (cv) m4 = ldg_f4(cv + c + q * 4);
+              const float4 m4 = ptx::lds_f4(wvec + (c + q * 4) * 4);
               const float mm[4] = {m4.x, m4.y, m4.z, m4.w};
 #pragma unroll
               for (int e = 0; e < 4; ++e) {
@@ -451,8 +535,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       const int groups = P.head_dim == 128 ? 1 : BLOCK_K / P.head_dim;  // heads per k-block
       for (int kb = 0; kb < P.num_kb; kb += step) {
         const int s0 = stage, s1 = (stage + 1) % STAGES;
-        ptx::mbar_wait(&bars->full[s0], phase);
-        if (step == 2) ptx::mbar_wait(&bars->full[s1], (s1 == 0) ? (phase ^ 1) : phase);
+        ptx::mbar_wait_suspend(&bars->full[s0], phase);
+        if (step == 2) ptx::mbar_wait_suspend(&bars->full[s1], (s1 == 0) ? (phase ^ 1) : phase);
         uint8_t* ra = smem_a + s0 * A_STAGE_BYTES + row_off;
         uint8_t* rb = step == 2 ? smem_a + s1 * A_STAGE_BYTES + row_off : ra;
         for (int gidx = 0; gidx < groups; ++gidx)
