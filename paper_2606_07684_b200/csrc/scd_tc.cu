@@ -136,6 +136,26 @@ __device__ __forceinline__ void stg_copy_out(uint32_t stg, int pitch, int row_by
   }
 }
 
+// packed fp32 pairs (FFMA2 / FMUL2 on sm_100a): half the FMA-pipe instructions of the epilogue
+__device__ __forceinline__ unsigned long long f2_pack(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
 __device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
 // RoPE epilogue of one K tile, specialised for HALF pairing, head_dim 128, 256-column tiles (two
@@ -147,9 +167,16 @@ __device__ __forceinline__ void rope_tile_h128(const TcParams& P, uint32_t t_row
                                                float rs, int lane) {
 #pragma unroll
   for (int jj = 0; jj < 32; jj += 16) {
-    float2 cs[16];
+    // (cos, cos), (sin, sin), (-sin, -sin) packed over adjacent frequency pairs
+    unsigned long long c2[8], s2[8], ns2[8];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) cs[i] = rope_cs(pos, P.rope_g[JG * 32 + jj + i]);
+    for (int i = 0; i < 8; ++i) {
+      const float2 x = rope_cs(pos, P.rope_g[JG * 32 + jj + 2 * i]), y = rope_cs(pos, P.rope_g[JG * 32 + jj + 2 * i + 1]);
+      c2[i] = f2_pack(x.x, y.x);
+      s2[i] = f2_pack(x.y, y.y);
+      ns2[i] = f2_pack(-x.y, -y.y);
+    }
+    const unsigned long long rs2 = f2_pack(rs, rs);
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       uint32_t ra[16], rb[16];
@@ -161,18 +188,19 @@ __device__ __forceinline__ void rope_tile_h128(const TcParams& P, uint32_t t_row
 #pragma unroll
       for (int q = 0; q < 4; ++q) {
         const float4 ma = ptx::lds_f4(wvec + (ca + q * 4) * 4), mb = ptx::lds_f4(wvec + (ca + 64 + q * 4) * 4);
-        const float am[4] = {ma.x, ma.y, ma.z, ma.w}, bm[4] = {mb.x, mb.y, mb.z, mb.w};
-        float va[4], vb[4];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          const int i = q * 4 + e;
-          const float a = fmaf(__uint_as_float(ra[i]), rs, am[e]);
-          const float b = fmaf(__uint_as_float(rb[i]), rs, bm[e]);
-          va[e] = a * cs[i].x - b * cs[i].y;
-          vb[e] = b * cs[i].x + a * cs[i].y;
+        for (int e = 0; e < 2; ++e) {
+          const int i = q * 4 + e * 2;                 // elements i, i + 1
+          const unsigned long long a = f2_fma(f2_pack(__uint_as_float(ra[i]), __uint_as_float(ra[i + 1])), rs2,
+                                              e ? f2_pack(ma.z, ma.w) : f2_pack(ma.x, ma.y));
+          const unsigned long long b = f2_fma(f2_pack(__uint_as_float(rb[i]), __uint_as_float(rb[i + 1])), rs2,
+                                              e ? f2_pack(mb.z, mb.w) : f2_pack(mb.x, mb.y));
+          float x0, x1, y0, y1;
+          f2_unpack(f2_fma(b, ns2[i >> 1], f2_mul(a, c2[i >> 1])), x0, x1);   // a cos - b sin
+          f2_unpack(f2_fma(a, s2[i >> 1], f2_mul(b, c2[i >> 1])), y0, y1);    // b cos + a sin
+          oa[q * 2 + e] = pack_bf16x2(x0, x1);
+          ob[q * 2 + e] = pack_bf16x2(y0, y1);
         }
-        oa[q * 2] = pack_bf16x2(va[0], va[1]); oa[q * 2 + 1] = pack_bf16x2(va[2], va[3]);
-        ob[q * 2] = pack_bf16x2(vb[0], vb[1]); ob[q * 2 + 1] = pack_bf16x2(vb[2], vb[3]);
       }
       const int k0 = h * 8 + (jj >> 3);               // chunk of run (h, a); run (h, b) = +4
       stg_put(stg, 256, lane, k0, make_uint4(oa[0], oa[1], oa[2], oa[3]));
@@ -292,19 +320,63 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   } else if (warp >= 4 && warp < 4 + EPI_WARPS) {
     // ============================== epilogue ==============================
     // One token row per thread (TMEM lane); warps w and w+4 share a lane quadrant and split the
-    // tile's columns into two groups.  Each group is processed in sub-tiles of <= 128 columns:
-    // TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced stores.
+    // tile's work into two groups (columns, or RoPE frequencies for 2-head K tiles).  Per group:
+    // TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced 16-B stores.
+    // The per-row quantities of the NEXT tile (position, slot, scales, mean slice) are fetched
+    // while the current tile is processed.
     const int ew = (warp - 4) & 3;                    // TMEM lane quadrant (= warp % 4)
-    const int grp = (warp - 4) >> 2;                  // column group 0 / 1
+    const int grp = (warp - 4) >> 2;                  // group 0 / 1
     const int half = P.head_dim / 2;
     const uint32_t stg = ptx::smem_u32(smem_stg + (warp - 4) * STG_WARP_BYTES);
     const uint32_t wvec = ptx::smem_u32(smem_vec + (warp - 4) * VEC_WARP_BYTES);
-    // split only when both halves keep whole heads (RoPE) and whole 32-column TMEM chunks
+    const int out_eb = (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2;
+    // column split only when both halves keep whole heads (RoPE) and whole 32-column TMEM chunks
     const int gran = (EPI == EPI_KV && P.head_dim > 32) ? P.head_dim : 32;
     const bool split_cols = (block_n % (2 * gran)) == 0;
     const int grp_cols = split_cols ? block_n / 2 : block_n;
-    const int out_eb = (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2;
+
+    struct RowInfo {
+      int pos;
+      float rs;
+      unsigned long long row_ptr;                     // global address of this row's first tile column (0 = no row)
+      float4 m0, m1;                                  // this lane's share of the tile's mean / bias slice
+    };
+    auto fetch = [&](int tile) -> RowInfo {
+      RowInfo ri;
+      ri.pos = 0; ri.rs = 1.0f; ri.row_ptr = 0ull;
+      ri.m0 = make_float4(0.f, 0.f, 0.f, 0.f); ri.m1 = ri.m0;
+      const int m_tile = tile % P.m_tiles;
+      const int n_tile = (tile / P.m_tiles) % P.n_tiles;
+      const TcSeg& sg = P.segs[tile / (P.m_tiles * P.n_tiles)];
+      const int row = m_tile * BLOCK_M + ew * 32 + lane;
+      const int n0 = n_tile * block_n;
+      if (sg.col_vec) {
+        ri.m0 = ldg_f4(sg.col_vec + n0 + lane * 4);
+        if (block_n > 128) ri.m1 = ldg_f4(sg.col_vec + n0 + 128 + lane * 4);
+      }
+      if (row < P.M) {
+        if (EPI == EPI_KV) {
+          long long slot;
+          row_to_pos_slot(P.batch, row, ri.pos, slot);
+          const bool to1 = n0 >= P.split;
+          ri.row_ptr = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
+                       ((unsigned long long)slot * P.pool_width + (to1 ? n0 - P.split : n0)) * 2ull;
+        } else {
+          ri.row_ptr = (unsigned long long)sg.out0 + ((unsigned long long)row * P.N + n0) * (unsigned long long)out_eb;
+        }
+        if ((EPI == EPI_KV || EPI == EPI_ACT) && sg.a_scale) ri.rs = __ldg(sg.a_scale + row);
+        if (EPI == EPI_KV && sg.rowscale_in) {
+          float ss = 0.0f;
+          for (int p = 0; p < P.n_partials; ++p) ss += __ldg(sg.rowscale_in + (size_t)p * P.M + row);
+          ri.rs *= rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
+        }
+      }
+      return ri;
+    };
+
     int it = 0;
+    RowInfo cur;
+    if ((int)blockIdx.x < total_tiles) cur = fetch(blockIdx.x);
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
       const int m_tile = tile % P.m_tiles;
       const int n_tile = (tile / P.m_tiles) % P.n_tiles;
@@ -318,46 +390,42 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       const int g_begin = grp * grp_cols;                     // this warp's columns [g_begin, g_end) of the tile
       const int g_end = min(n_end, g_begin + grp_cols);
       const bool has_work = (grp == 0 || split_cols) && g_begin < n_end;
+      const int pos = cur.pos;
+      const float rs = cur.rs;
+      const unsigned long long row_ptr = cur.row_ptr;
 
-      // ---- per-row quantities (issued before waiting for the accumulator) ----
-      int pos = 0;
-      float rs = 1.0f;
-      unsigned long long row_ptr = 0ull;                      // global address of this row's first tile column
-      if (valid) {
-        if (EPI == EPI_KV) {
-          long long slot;
-          row_to_pos_slot(P.batch, row, pos, slot);
-          const bool to1 = n0 >= P.split;
-          row_ptr = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
-                    ((unsigned long long)slot * P.pool_width + (to1 ? n0 - P.split : n0)) * 2ull;
-        } else {
-          row_ptr = (unsigned long long)sg.out0 + ((unsigned long long)row * P.N + n0) * (unsigned long long)out_eb;
-        }
-        if ((EPI == EPI_KV || EPI == EPI_ACT) && sg.a_scale) rs = __ldg(sg.a_scale + row);
-        if (EPI == EPI_KV && sg.rowscale_in) {
-          float ss = 0.0f;
-          for (int p = 0; p < P.n_partials; ++p) ss += __ldg(sg.rowscale_in + (size_t)p * P.M + row);
-          rs *= rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
-        }
-      }
-      // this warp's copy of the tile's mean / bias slice (zeros when absent): wvec[c] for tile column c
-      {
-        float4 m0 = make_float4(0.f, 0.f, 0.f, 0.f), m1 = m0;
-        if (sg.col_vec) {
-          m0 = ldg_f4(sg.col_vec + n0 + lane * 4);
-          if (block_n > 128) m1 = ldg_f4(sg.col_vec + n0 + 128 + lane * 4);
-        }
-        __syncwarp();
-        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(m0.x), "f"(m0.y), "f"(m0.z), "f"(m0.w) : "memory");
-        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + 512 + lane * 16), "f"(m1.x), "f"(m1.y), "f"(m1.z), "f"(m1.w) : "memory");
-        __syncwarp();
-      }
+      // this warp's copy of the tile's mean / bias slice: wvec[c] for tile column c
+      __syncwarp();
+      asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(cur.m0.x), "f"(cur.m0.y),
+                   "f"(cur.m0.z), "f"(cur.m0.w) : "memory");
+      asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + 512 + lane * 16), "f"(cur.m1.x), "f"(cur.m1.y),
+                   "f"(cur.m1.z), "f"(cur.m1.w) : "memory");
+      __syncwarp();
 
       ptx::mbar_wait_suspend(&bars->tmem_full[acc], acc_phase);
       ptx::tc_fence_after();
       const uint32_t t_row = tmem_base + (uint32_t)(acc * block_n) + ((uint32_t)(ew * 32) << 16);
 
-      // e4m3 codes: the row scale needs the amax over all of N first (tile spans N)
+      // prefetch the next tile's per-row quantities; consumed at the bottom of the loop
+      RowInfo nxt = cur;
+      if (tile + (int)gridDim.x < total_tiles) nxt = fetch(tile + gridDim.x);
+
+      if (EPI == EPI_KV && n0 < sg.rope_cols && P.rope_style == SCD_ROPE_HALF && P.head_dim == 128 && block_n == 256 &&
+          n_end == 256) {
+        // ---- 2-head K tile: frequency split between the warp pair ----
+        if (grp == 0) rope_tile_h128<0>(P, t_row, stg, wvec, pos, rs, lane);
+        else rope_tile_h128<1>(P, t_row, stg, wvec, pos, rs, lane);
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+        if (grp == 0) rope_tile_h128_copy_out<0>(stg, row_ptr, lane);
+        else rope_tile_h128_copy_out<1>(stg, row_ptr, lane);
+        cur = nxt;
+        continue;
+      }
+
+      // e4m3 codes: the row scale needs the amax over all of N first (tile spans N).  Columns
+      // beyond N hold acc = 0 (zero-filled operand rows) and c = 0 (padded vector): no masks needed.
       float e4_scale = 1.0f;
       if (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE && has_work) {
         float amax = 0.0f;
@@ -368,10 +436,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 #pragma unroll
           for (int q = 0; q < 8; ++q) {
             const float4 m4 = ptx::lds_f4(wvec + (c + q * 4) * 4);
-            const float mm[4] = {m4.x, m4.y, m4.z, m4.w};
-#pragma unroll
-            for (int e = 0; e < 4; ++e)
-              if (c + q * 4 + e < n_end) amax = fmaxf(amax, fabsf(__uint_as_float(r[q * 4 + e]) - mm[e]));
+            amax = fmaxf(amax, fmaxf(fmaxf(fabsf(__uint_as_float(r[q * 4]) - m4.x), fabsf(__uint_as_float(r[q * 4 + 1]) - m4.y)),
+                                     fmaxf(fabsf(__uint_as_float(r[q * 4 + 2]) - m4.z), fabsf(__uint_as_float(r[q * 4 + 3]) - m4.w))));
           }
         }
         e4_scale = amax > 0.0f ? amax / 448.0f : 1.0f;
@@ -379,23 +445,12 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       }
       float ss_u = 0.0f;
 
-      if (EPI == EPI_KV && n0 < sg.rope_cols && P.rope_style == SCD_ROPE_HALF && P.head_dim == 128 && block_n == 256 &&
-          n_end == 256) {
-        if (grp == 0) rope_tile_h128<0>(P, t_row, stg, wvec, pos, rs, lane);
-        else rope_tile_h128<1>(P, t_row, stg, wvec, pos, rs, lane);
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
-        if (grp == 0) rope_tile_h128_copy_out<0>(stg, row_ptr, lane);
-        else rope_tile_h128_copy_out<1>(stg, row_ptr, lane);
-        __syncwarp();
-        continue;
-      }
       if (!has_work) {                                        // nothing to read: release the accumulator
         if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = 0.0f;
         ptx::tc_fence_before();
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+        cur = nxt;
         continue;
       }
       for (int c0 = g_begin; c0 < g_end; c0 += SUB_N) {
@@ -405,7 +460,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         const bool last_sub = c0 + SUB_N >= g_end;
 
         if (EPI == EPI_KV && (n0 + c0) < sg.rope_cols && P.rope_style == SCD_ROPE_HALF) {
-          // ---- RoPE, HALF pairing: heads of this sub-tile, 16 pairs at a time ----
+          // ---- RoPE, HALF pairing (generic): heads of this sub-tile, 16 pairs at a time ----
           for (int hc = 0; hc < sub_cols; hc += P.head_dim)
             for (int j0 = 0; j0 < half; j0 += 16) {
               uint32_t ra[16], rb[16];
@@ -439,6 +494,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
             }
         } else {
           // ---- 32 columns at a time: plain epilogues, or INTERLEAVED RoPE (adjacent pairs) ----
+          const unsigned long long rs2 = f2_pack(rs, rs);
           for (int c = c0; c < c0 + sub_cols; c += 32) {
             uint32_t r[32];
             ptx::tmem_ld32(t_row + c, r);
@@ -447,18 +503,23 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
               const float4 m4 = ptx::lds_f4(wvec + (c + q * 4) * 4);
-              const float mm[4] = {m4.x, m4.y, m4.z, m4.w};
-#pragma unroll
-              for (int e = 0; e < 4; ++e) {
-                const int i = q * 4 + e;
-                float x = __uint_as_float(r[i]);
-                if (EPI == EPI_CODES) x -= mm[e];
-                else x = fmaf(x, rs, mm[e]);
-                if (EPI == EPI_ACT && P.act == SCD_ACT_SILU) x = __fdividef(x, 1.0f + __expf(-x));
-                if (c + i >= n_end) x = 0.0f;
-                if (EPI == EPI_U) ss_u = fmaf(x, x, ss_u);
-                v[i] = x;
+              if (EPI == EPI_CODES) {
+                v[q * 4] = __uint_as_float(r[q * 4]) - m4.x; v[q * 4 + 1] = __uint_as_float(r[q * 4 + 1]) - m4.y;
+                v[q * 4 + 2] = __uint_as_float(r[q * 4 + 2]) - m4.z; v[q * 4 + 3] = __uint_as_float(r[q * 4 + 3]) - m4.w;
+              } else {
+                f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4]), __uint_as_float(r[q * 4 + 1])), rs2, f2_pack(m4.x, m4.y)),
+                          v[q * 4], v[q * 4 + 1]);
+                f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4 + 2]), __uint_as_float(r[q * 4 + 3])), rs2, f2_pack(m4.z, m4.w)),
+                          v[q * 4 + 2], v[q * 4 + 3]);
               }
+            }
+            if (EPI == EPI_ACT && P.act == SCD_ACT_SILU) {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) v[i] = __fdividef(v[i], 1.0f + __expf(-v[i]));
+            }
+            if (EPI == EPI_U) {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) ss_u = fmaf(v[i], v[i], ss_u);
             }
             if (EPI == EPI_KV && (n0 + c) < sg.rope_cols) {
               const int f0 = ((n0 + c) % P.head_dim) >> 1;
@@ -505,6 +566,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         __syncwarp();
       }
       if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = ss_u;
+      cur = nxt;
     }
   } else if (AMODE == A_DEROPE && warp >= 4 + EPI_WARPS) {
     // ============================== A transform: deRoPE in shared memory ==============================
