@@ -170,6 +170,24 @@ def run_reference(args, cfg):
     print(json.dumps(line))
 
 
+# ------------------------------------------------------------------------------ rank aggregation
+def reduce_max_over_ranks(values, device="cpu"):
+    """Element-wise MAX over ranks (times are reported as the slowest rank's); identity when
+    torch.distributed is not initialised.  Works on gloo (CPU tests) and nccl."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+def whole_job_throughput(tokens_per_rank: int, world: int, step_ms_max: float) -> float:
+    """Replicas only: every rank rebuilds `tokens_per_rank` tokens per step; the job's rate is all
+    ranks' tokens over the slowest rank's step time."""
+    return tokens_per_rank * world / (step_ms_max * 1e-3)
+
+
 # ------------------------------------------------------------------------------ our arm
 def run_ours(args, cfg):
     import torch
@@ -284,10 +302,8 @@ def run_ours(args, cfg):
     clocks = sampler.stop() if sampler else None
 
     # ---- max over ranks ----
-    vals = torch.tensor([step_ms, enc_ms, dec_ms, pat_ms, e2e["ms"] if e2e else 0.0], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
-    step_ms, enc_ms, dec_ms, pat_ms, e2e_ms = vals.tolist()
+    step_ms, enc_ms, dec_ms, pat_ms, e2e_ms = reduce_max_over_ranks(
+        [step_ms, enc_ms, dec_ms, pat_ms, e2e["ms"] if e2e else 0.0], dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -297,11 +313,14 @@ def run_ours(args, cfg):
     costs = workload_costs(cfg, T)
     # DRAM bytes per launch from the committed `ncu --set full` captures (profiles/): {kernel: bytes}
     traffic = {}
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(tpath):
-        traffic = json.load(open(tpath)).get(cfg.name, {})
+        for ln in open(tpath).read().splitlines()[1:]:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 3 and f[0] == cfg.name:
+                traffic[f[1]] = float(f[2])
     tokens = T * world
-    value = tokens / (step_ms * 1e-3)
+    value = whole_job_throughput(T, world, step_ms)
 
     # dominant kernel of the step = largest total time over the profiled passes
     tot = {kid: sum(v_) for kid, v_ in by_kernel.items()}
@@ -390,7 +409,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", default="llama3_8b_8k")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--ref-rows", type=int, default=256)
+    ap.add_argument("--ref-rows", type=int, default=4096)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
