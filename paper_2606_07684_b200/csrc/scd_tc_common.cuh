@@ -1,0 +1,89 @@
+// Shared between the tcgen05 kernels (scd_tc.cu: generic GEMM + epilogues; scd_tc_kv.cu: the
+// paged-KV specialisation): kernel parameters, tile constants, small device helpers.
+#pragma once
+
+#include <cuda_fp16.h>
+
+#include "ptx.cuh"
+#include "scd_device.cuh"
+#include "scd_tc.h"
+
+namespace scd {
+
+// ---------------------------------------------------------------------------------
+// kernel parameters
+// ---------------------------------------------------------------------------------
+struct TcSeg {
+  const float* col_vec;      // EPI_CODES: c[n] (subtracted); else mean / bias [N] (added)
+  const float* a_scale;      // row scales of e4m3 codes used as A (null otherwise)
+  void* out0;
+  void* out1;
+  float* aux;
+  const float* rowscale_in;  // NORM_RMS: sum-of-squares partials [n_partials][M]
+  int32_t a_map, a_z, b_map, rope_cols;
+};
+
+struct TcParams {
+  CUtensorMap a_maps[TC_MAX_AMAPS];
+  TcSeg segs[TC_MAX_SEGS];
+  uint32_t rope_g[64];                // theta^(-2j/d_h) / (2 pi) as a Q0.32 fraction of a turn
+  const CUtensorMap* b_maps;          // plan-owned, global memory
+  BatchDev batch;
+  int32_t n_segs, M, N, K;
+  int32_t m_tiles, n_tiles, num_kb, block_n, stages;
+  int32_t a_kb_per_head;              // >0: A is [T, H, d_h] head-strided, k-blocks per head
+  int32_t split, pool_width, head_dim, rope_style, act, code_dtype;
+  int32_t n_partials, rms_dim;
+  float rms_eps;
+};
+
+constexpr int BLOCK_M = 128, BLOCK_K = 64, MAX_STAGES = 8, TMEM_COLS = 512;
+constexpr int EPI_WARPS = 8;                                // two per TMEM lane quadrant, splitting the columns
+constexpr int A_STAGE_BYTES = BLOCK_M * BLOCK_K * 2;        // 16 KB
+constexpr int SUB_N = 128;                                  // epilogue sub-tile width (columns)
+constexpr int STG_WARP_BYTES = 32 * SUB_N * 2;              // per-warp staging: 32 rows x 256 B
+constexpr int VEC_WARP_BYTES = 256 * 4;                     // per-warp copy of the tile's mean / bias slice
+
+
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
+
+// (cos, sin) of position * theta^(-2j/d_h).  The angle is tracked as a 32-bit fraction of a
+// turn: pos * g wraps modulo 2^32 exactly, so the reduced angle in [-pi, pi) has an absolute
+// error <= pos * 2 pi * 2^-33 + 2^-24 turn (2.4e-5 rad at 32k positions) before the MUFU
+// approximations (2^-21 abs).  No table, no memory traffic.
+__device__ __forceinline__ float2 rope_cs(int pos, uint32_t g) {
+  const float x = (float)(int32_t)((uint32_t)pos * g) * 1.4629180792671596e-9f;   // 2 pi / 2^32
+  return make_float2(__cosf(x), __sinf(x));
+}
+
+// packed fp32 pairs (FFMA2 / FMUL2 on sm_100a): half the FMA-pipe instructions of the epilogue
+__device__ __forceinline__ unsigned long long f2_pack(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+
+__device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+
+// scd_tc_kv.cu: can the specialised paged-KV kernel take this launch?  (head_dim 128, HALF RoPE,
+// 256-column tiles, whole tiles only.)  P.M/N/K/block_n/split/rope fields must be filled.
+bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P);
+scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s);
+
+}  // namespace scd

@@ -1,0 +1,384 @@
+// Paged-KV specialisation of the tcgen05 GEMM: REUSE decode (Eq. 9) and PATCH
+// GEMM-3 (Eq. 12a/b) for head_dim 128, HALF RoPE, 256-column (two-head) tiles.
+//
+// Same TMA -> tcgen05 -> TMEM main loop as scd_tc.cu; what differs is the tile order and the epilogue,
+// which is where this kernel's time goes (it writes 8x what it reads):
+//
+//   * tiles are walked m-slowest (m-tile, segment, n-tile) and each CTA owns one contiguous range, so
+//     a CTA sees at most a handful of m-tiles: the per-row quantities (position, slot, RMS scale) and
+//     the row's (cos, sin) are computed when the m-tile changes and then live in registers;
+//   * 16 epilogue warps: warp (q, g) owns TMEM lane quadrant q (32 token rows, one per lane) and,
+//     for K tiles, RoPE frequencies [16g, 16g+16) of both heads -- every (cos, sin) is used for two
+//     heads and for every layer of the m-tile; for V tiles, columns [64g, 64g+64);
+//   * the four warps of a quadrant stage bf16 results in one swizzled [32 x 512 B] buffer, meet at a
+//     named barrier, and each copies 8 complete 512-B row segments to the rows' slots of the paged
+//     pool with fully coalesced 16-B stores.
+#include <algorithm>
+#include <cstring>
+
+#include "scd_tc_common.cuh"
+
+namespace scd {
+
+namespace {
+
+constexpr int KV_BLOCK_N = 256;
+constexpr int KV_EPI_WARPS = 16;
+constexpr int KV_B_STAGE_BYTES = KV_BLOCK_N * BLOCK_K * 2;   // 32 KB
+constexpr int KV_STG_BYTES = 4 * 32 * KV_BLOCK_N * 2;        // 4 quadrants x [32 rows x 512 B] = 64 KB
+constexpr int KV_VEC_BYTES = KV_EPI_WARPS * 64 * 4;          // per-warp slice of the tile's mean / bias: 64 floats
+
+struct __align__(8) KvBarriers {
+  uint64_t full[MAX_STAGES], empty[MAX_STAGES];
+  uint64_t tmem_full[2], tmem_empty[2];
+  uint32_t tmem_base;
+};
+
+size_t kv_smem_bytes(int stages) {
+  return 1024 + (size_t)stages * (A_STAGE_BYTES + KV_B_STAGE_BYTES) + KV_STG_BYTES + KV_VEC_BYTES + sizeof(KvBarriers);
+}
+int kv_pick_stages(int num_kb) {
+  const size_t budget = 232448 - 1024 - KV_STG_BYTES - KV_VEC_BYTES - sizeof(KvBarriers);
+  int st = (int)(budget / (A_STAGE_BYTES + KV_B_STAGE_BYTES));
+  if (st > MAX_STAGES) st = MAX_STAGES;
+  if (st > 2 * num_kb) st = 2 * num_kb;
+  return st < 2 ? 2 : st;
+}
+
+// quadrant staging buffer: 32 rows x 512 B, 16-byte chunks XOR-swizzled with the row's low 3 bits:
+// row-per-lane writes and row-per-warp reads are both conflict free
+__device__ __forceinline__ uint32_t qstg_addr(uint32_t stg, int row, int chunk) {
+  return stg + row * 512 + (((chunk & ~7) | ((chunk ^ row) & 7)) << 4);
+}
+
+struct TileCoord {
+  int m_tile, seg, n_tile;
+};
+__device__ __forceinline__ TileCoord tile_coord(const TcParams& P, int tile) {
+  const int per_m = P.n_segs * P.n_tiles;
+  TileCoord c;
+  c.m_tile = tile / per_m;
+  const int rem = tile - c.m_tile * per_m;
+  c.seg = rem / P.n_tiles;
+  c.n_tile = rem - c.seg * P.n_tiles;
+  return c;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------
+// the kernel: warp 0 = TMEM allocator + TMA producer, warp 1 = MMA issuer, warps 2-3 idle, warps 4..19 =
+// epilogue.  Registers live per SM sub-partition (16 K each, 5 warps): warpgroup 0 shrinks to 32 registers so
+// that the four epilogue warps of each sub-partition can hold 112 (setmaxnreg).
+// ---------------------------------------------------------------------------------
+constexpr int KV_FIRST_EPI_WARP = 4;
+constexpr int KV_NTHREADS = (KV_FIRST_EPI_WARP + KV_EPI_WARPS) * 32;   // 640
+
+__global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  const int STAGES = P.stages;
+  uint8_t* smem_a = smem;
+  uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
+  uint8_t* smem_stg = smem_b + STAGES * KV_B_STAGE_BYTES;
+  uint8_t* smem_vec = smem_stg + KV_STG_BYTES;
+  KvBarriers* bars = (KvBarriers*)(smem_vec + KV_VEC_BYTES);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int total_tiles = P.m_tiles * P.n_segs * P.n_tiles;
+  const int t_begin = (int)((long long)total_tiles * blockIdx.x / gridDim.x);
+  const int t_end = (int)((long long)total_tiles * (blockIdx.x + 1) / gridDim.x);
+
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      ptx::mbar_init(&bars->full[s], 1);
+      ptx::mbar_init(&bars->empty[s], 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      ptx::mbar_init(&bars->tmem_full[a], 1);
+      ptx::mbar_init(&bars->tmem_empty[a], 4);          // one arrival per lane quadrant
+    }
+    ptx::fence_barrier_init();
+  }
+  if (warp == 0) {
+    ptx::tmem_alloc<TMEM_COLS>(&bars->tmem_base);
+    ptx::tmem_relinquish();
+  }
+  ptx::tc_fence_before();
+  __syncthreads();
+  ptx::tc_fence_after();
+  const uint32_t tmem_base = bars->tmem_base;
+
+  if (warp < KV_FIRST_EPI_WARP) {
+    ptx::setmaxnreg_dec<32>();   // 128 x 32 + 512 x 112 = 640 x 96: the CTA pool is what the launch allocated
+  if (warp == 0) {
+    // ============================== TMA producer ==============================
+    if (lane == 0) {
+      int stage = 0;
+      uint32_t phase = 0;
+      for (int tile = t_begin; tile < t_end; ++tile) {
+        const TileCoord tc = tile_coord(P, tile);
+        const TcSeg& sg = P.segs[tc.seg];
+        const CUtensorMap* am = &P.a_maps[sg.a_map];
+        const CUtensorMap* bm = P.b_maps + sg.b_map;
+        for (int kb = 0; kb < P.num_kb; ++kb) {
+          ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
+          ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES + KV_B_STAGE_BYTES);
+          ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES, am, &bars->full[stage], kb * BLOCK_K, tc.m_tile * BLOCK_M,
+                           sg.a_z);
+          ptx::tma_load_2d(smem_b + stage * KV_B_STAGE_BYTES, bm, &bars->full[stage], kb * BLOCK_K,
+                           tc.n_tile * KV_BLOCK_N);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ============================== MMA issuer ==============================
+    if (lane == 0) {
+      const uint32_t idesc = ptx::umma_idesc_bf16(BLOCK_M, KV_BLOCK_N);
+      int stage = 0;
+      uint32_t phase = 0;
+      int it = 0;
+      for (int tile = t_begin; tile < t_end; ++tile, ++it) {
+        const int acc = it & 1;
+        const uint32_t acc_phase = (it >> 1) & 1;
+        ptx::mbar_wait_suspend(&bars->tmem_empty[acc], acc_phase ^ 1);
+        ptx::tc_fence_after();
+        const uint32_t d_tmem = tmem_base + (uint32_t)(acc * KV_BLOCK_N);
+        for (int kb = 0; kb < P.num_kb; ++kb) {
+          ptx::mbar_wait_suspend(&bars->full[stage], phase);
+          ptx::tc_fence_after();
+          const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
+          const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * KV_B_STAGE_BYTES));
+#pragma unroll
+          for (int k = 0; k < BLOCK_K / 16; ++k)
+            ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb | k) != 0);
+          ptx::mma_commit(&bars->empty[stage]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        ptx::mma_commit(&bars->tmem_full[acc]);
+      }
+    }
+  }
+  } else {
+    // ============================== epilogue ==============================
+    ptx::setmaxnreg_inc<112>();
+    const int q = warp & 3;                                   // TMEM lane quadrant this warp may read
+    const int g = (warp - KV_FIRST_EPI_WARP) >> 2;            // frequency / column group 0..3
+    const uint32_t stg = ptx::smem_u32(smem_stg) + (uint32_t)q * (32 * 512);
+    const uint32_t wvec = ptx::smem_u32(smem_vec) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 256;
+    const uint32_t bar_id = 1 + q;
+
+    // per-row state, recomputed when the m-tile changes
+    int cur_m = -1;
+    unsigned long long slot_off = 0;                          // byte offset of the row's slot inside a pool
+    bool valid = false;
+    float rs_row = 1.0f;
+    unsigned long long c2[8], s2[8];                          // (cos, sin) of frequencies 16g + {2i, 2i+1}, packed pairs
+#pragma unroll
+    for (int i = 0; i < 8; ++i) c2[i] = s2[i] = 0ull;
+
+    // per-tile prefetch: this lane's float4 of the warp's mean / bias slice, e4m3 row scale
+    struct Pre {
+      float4 vec;
+      float a_scale;
+    };
+    auto fetch = [&](int tile) -> Pre {
+      Pre pr;
+      pr.vec = make_float4(0.f, 0.f, 0.f, 0.f);
+      pr.a_scale = 1.0f;
+      const TileCoord tc = tile_coord(P, tile);
+      const TcSeg& sg = P.segs[tc.seg];
+      const int n0 = tc.n_tile * KV_BLOCK_N;
+      if (sg.col_vec && lane < 16) {
+        const int run = lane >> 2, part = lane & 3;
+        const int col = (n0 < sg.rope_cols) ? (run >> 1) * 128 + (run & 1) * 64 + 16 * g + part * 4 : 64 * g + lane * 4;
+        pr.vec = ldg_f4(sg.col_vec + n0 + col);
+      }
+      if (sg.a_scale) {
+        const int row = tc.m_tile * BLOCK_M + q * 32 + lane;
+        if (row < P.M) pr.a_scale = __ldg(sg.a_scale + row);
+      }
+      return pr;
+    };
+
+    Pre cur;
+    if (t_begin < t_end) cur = fetch(t_begin);
+    int it = 0;
+    for (int tile = t_begin; tile < t_end; ++tile, ++it) {
+      const TileCoord tc = tile_coord(P, tile);
+      const TcSeg& sg = P.segs[tc.seg];
+      const int acc = it & 1;
+      const uint32_t acc_phase = (it >> 1) & 1;
+      const int n0 = tc.n_tile * KV_BLOCK_N;
+      const bool is_k = n0 < sg.rope_cols;
+
+      if (tc.m_tile != cur_m) {
+        cur_m = tc.m_tile;
+        const int row = cur_m * BLOCK_M + q * 32 + lane;
+        valid = row < P.M;
+        int pos = 0;
+        long long slot = 0;
+        rs_row = 1.0f;
+        if (valid) {
+          row_to_pos_slot(P.batch, row, pos, slot);
+          if (sg.rowscale_in) {                                 // NORM_RMS (PATCH GEMM-3; single segment)
+            float ss = 0.0f;
+            for (int p = 0; p < P.n_partials; ++p) ss += __ldg(sg.rowscale_in + (size_t)p * P.M + row);
+            rs_row = rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
+          }
+        }
+        slot_off = (unsigned long long)slot * (unsigned long long)P.pool_width * 2ull;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float2 x = rope_cs(pos, P.rope_g[16 * g + 2 * i]), y = rope_cs(pos, P.rope_g[16 * g + 2 * i + 1]);
+          c2[i] = f2_pack(x.x, y.x);
+          s2[i] = f2_pack(x.y, y.y);
+        }
+      }
+      const float rs = rs_row * cur.a_scale;
+      const unsigned long long rs2 = f2_pack(rs, rs);
+      const bool to1 = n0 >= P.split;
+      const unsigned long long row_base =
+          valid ? (unsigned long long)(to1 ? sg.out1 : sg.out0) + slot_off + (unsigned long long)(to1 ? n0 - P.split : n0) * 2ull
+                : 0ull;
+
+      // this warp's slice of the tile's mean / bias: wvec[16 * run + i]
+      __syncwarp();
+      if (lane < 16)
+        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(cur.vec.x), "f"(cur.vec.y),
+                     "f"(cur.vec.z), "f"(cur.vec.w) : "memory");
+      __syncwarp();
+
+      ptx::mbar_wait_suspend(&bars->tmem_full[acc], acc_phase);
+      ptx::tc_fence_after();
+      const uint32_t t_row = tmem_base + (uint32_t)(acc * KV_BLOCK_N) + ((uint32_t)(q * 32) << 16);
+
+      Pre nxt = cur;
+      if (tile + 1 < t_end) nxt = fetch(tile + 1);
+
+      if (is_k) {
+        // ---- K tile: rotate pairs (j, j + 64) of both heads, j in [16g, 16g + 16) ----
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          uint32_t ra[16], rb[16];
+          const int ca = h * 128 + 16 * g;
+          ptx::tmem_ld16(t_row + ca, ra);
+          ptx::tmem_ld16(t_row + ca + 64, rb);
+          ptx::tmem_ld_wait();
+          uint32_t oa[8], ob[8];
+#pragma unroll
+          for (int q4 = 0; q4 < 4; ++q4) {
+            const float4 ma = ptx::lds_f4(wvec + ((2 * h) * 16 + q4 * 4) * 4);
+            const float4 mb = ptx::lds_f4(wvec + ((2 * h + 1) * 16 + q4 * 4) * 4);
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+              const int i = q4 * 4 + e * 2, k = q4 * 2 + e;
+              const unsigned long long a = f2_fma(f2_pack(__uint_as_float(ra[i]), __uint_as_float(ra[i + 1])), rs2,
+                                                  e ? f2_pack(ma.z, ma.w) : f2_pack(ma.x, ma.y));
+              const unsigned long long b = f2_fma(f2_pack(__uint_as_float(rb[i]), __uint_as_float(rb[i + 1])), rs2,
+                                                  e ? f2_pack(mb.z, mb.w) : f2_pack(mb.x, mb.y));
+              float x0, x1, y0, y1, t0, t1;
+              f2_unpack(f2_mul(b, s2[k]), t0, t1);
+              f2_unpack(f2_fma(a, c2[k], f2_pack(-t0, -t1)), x0, x1);     // a cos - b sin
+              f2_unpack(f2_fma(a, s2[k], f2_mul(b, c2[k])), y0, y1);      // b cos + a sin
+              oa[k] = pack_bf16x2(x0, x1);
+              ob[k] = pack_bf16x2(y0, y1);
+            }
+          }
+          if (h == 0) ptx::named_bar_sync(bar_id, 128);         // the quadrant's previous copy-out has drained
+          const int k0 = h * 16 + 2 * g;                        // 16-B chunk of run (h, a); run (h, b) = +8
+          ptx::sts128(qstg_addr(stg, lane, k0), make_uint4(oa[0], oa[1], oa[2], oa[3]));
+          ptx::sts128(qstg_addr(stg, lane, k0 + 1), make_uint4(oa[4], oa[5], oa[6], oa[7]));
+          ptx::sts128(qstg_addr(stg, lane, k0 + 8), make_uint4(ob[0], ob[1], ob[2], ob[3]));
+          ptx::sts128(qstg_addr(stg, lane, k0 + 9), make_uint4(ob[4], ob[5], ob[6], ob[7]));
+        }
+      } else {
+        // ---- V tile (or K without RoPE): columns [64g, 64g + 64), 32 at a time ----
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          uint32_t r[32];
+          ptx::tmem_ld32(t_row + 64 * g + 32 * c, r);
+          ptx::tmem_ld_wait();
+          uint32_t o[16];
+#pragma unroll
+          for (int q4 = 0; q4 < 8; ++q4) {
+            const float4 m4 = ptx::lds_f4(wvec + (c * 32 + q4 * 4) * 4);
+            float v0, v1, v2, v3;
+            f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q4 * 4]), __uint_as_float(r[q4 * 4 + 1])), rs2, f2_pack(m4.x, m4.y)), v0, v1);
+            f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q4 * 4 + 2]), __uint_as_float(r[q4 * 4 + 3])), rs2, f2_pack(m4.z, m4.w)), v2, v3);
+            o[q4 * 2] = pack_bf16x2(v0, v1);
+            o[q4 * 2 + 1] = pack_bf16x2(v2, v3);
+          }
+          if (c == 0) ptx::named_bar_sync(bar_id, 128);
+          const int k0 = 8 * g + 4 * c;
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            ptx::sts128(qstg_addr(stg, lane, k0 + j), make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]));
+        }
+      }
+      // staging complete and all TMEM reads of the quadrant done: hand the accumulator back, copy out
+      ptx::tc_fence_before();
+      ptx::named_bar_sync(bar_id, 128);
+      if (g == 0 && lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+      {
+        uint4 v[8];
+        unsigned long long base[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const int r = 8 * g + i;
+          base[i] = __shfl_sync(0xffffffffu, row_base, r);
+          v[i] = ptx::lds128(qstg_addr(stg, r, lane));
+        }
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          if (base[i] != 0ull) ptx::stg128(base[i] + (unsigned long long)lane * 16ull, v[i]);
+      }
+      cur = nxt;
+    }
+  }
+
+  // ============================== teardown ==============================
+  ptx::tc_fence_before();
+  __syncthreads();
+  if (warp == 0) ptx::tmem_dealloc<TMEM_COLS>(tmem_base);
+}
+
+// ---------------------------------------------------------------------------------
+// host side
+// ---------------------------------------------------------------------------------
+bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P) {
+  if (p->model.head_dim != 128 || p->model.rope_style != SCD_ROPE_HALF) return false;
+  if (P.block_n != KV_BLOCK_N || (P.N % KV_BLOCK_N) || (P.split % KV_BLOCK_N) || P.a_kb_per_head != 0) return false;
+  for (int i = 0; i < P.n_segs; ++i) {
+    if (P.segs[i].rope_cols % KV_BLOCK_N) return false;
+    if (P.segs[i].rowscale_in && P.n_segs != 1) return false;
+  }
+  return true;
+}
+
+scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
+  P.m_tiles = (P.M + BLOCK_M - 1) / BLOCK_M;
+  P.n_tiles = P.N / KV_BLOCK_N;
+  P.num_kb = (P.K + BLOCK_K - 1) / BLOCK_K;
+  const int total = P.n_segs * P.m_tiles * P.n_tiles;
+  if (total <= 0) return SCD_OK;
+  P.stages = kv_pick_stages(P.num_kb);
+  const size_t smem = kv_smem_bytes(P.stages);
+  static thread_local size_t configured = 0;
+  if (configured < smem) {
+    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
+    configured = smem;
+  }
+  const int grid = std::min(total, p->sm_count);
+  prof_begin(s);
+  tc_kv_kernel<<<grid, KV_NTHREADS, smem, s>>>(P);
+  prof_end(s, 100 + 10 * EPI_KV);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_kv_kernel launch: %s", cudaGetErrorString(e));
+  count_launch();
+  return SCD_OK;
+}
+
+}  // namespace scd
