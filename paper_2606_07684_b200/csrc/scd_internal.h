@@ -8,6 +8,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <atomic>
 #include <vector>
 
 #include "scd.h"
@@ -112,6 +113,10 @@ struct scd_plan {
   // tcgen05 path: plan-owned TMA descriptors of the B operands in device memory
   // ([0,nseg) encoders, [nseg,2nseg) decoders, then 3 per PATCH layer)
   void* tc_bmaps = nullptr;
+  // tile-scheduler counters of the persistent paged-KV kernel: KV_SCHED_SETS pairs {next chunk, CTAs done},
+  // zero between launches (the last CTA of a launch resets its pair); launches take the sets round-robin
+  int32_t* kv_sched = nullptr;
+  mutable std::atomic<uint32_t> kv_sched_next{0};
 };
 
 namespace scd {

@@ -671,6 +671,11 @@ scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
   if (cudaMemcpy(d, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess)
     return fail(SCD_E_CUDA, "cudaMemcpy(tensor maps)");
   p->tc_bmaps = d;
+  void* sc = nullptr;
+  if (cudaMalloc(&sc, KV_SCHED_SETS * 2 * sizeof(int32_t)) != cudaSuccess) return fail(SCD_E_NOMEM, "cudaMalloc(kv scheduler)");
+  p->allocs.push_back(sc);
+  if (cudaMemset(sc, 0, KV_SCHED_SETS * 2 * sizeof(int32_t)) != cudaSuccess) return fail(SCD_E_CUDA, "cudaMemset(kv scheduler)");
+  p->kv_sched = (int32_t*)sc;
 
   (void)s;
   return SCD_OK;
@@ -857,7 +862,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
           return st;
       }
     }
-    if ((st = tc_kv_eligible(p, P) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
+    if ((st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     i = j;
   }
   (void)soff;
@@ -903,7 +908,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     P.segs[0].col_vec = pp.bkv; P.segs[0].out0 = kv->k_pool[pp.layer]; P.segs[0].out1 = kv->v_pool[pp.layer];
     P.segs[0].rowscale_in = rms ? ws_ss : nullptr; P.segs[0].rope_cols = D;
     P.segs[0].b_map = 2 * nseg + 3 * (int)j + 2;
-    if ((st = tc_kv_eligible(p, P) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
+    if ((st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
   }
   (void)soff;
   return SCD_OK;

@@ -35,8 +35,12 @@ struct TcParams {
   int32_t split, pool_width, head_dim, rope_style, act, code_dtype;
   int32_t n_partials, rms_dim;
   float rms_eps;
+  int32_t* sched;                     // paged-KV kernel: {next chunk, CTAs done}
+  int32_t chunk_tiles, n_chunks;      // paged-KV kernel: consecutive tiles per dynamically claimed unit
+  int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
 };
 
+constexpr int KV_SCHED_SETS = 64;
 constexpr int BLOCK_M = 128, BLOCK_K = 64, MAX_STAGES = 8, TMEM_COLS = 512;
 constexpr int EPI_WARPS = 8;                                // two per TMEM lane quadrant, splitting the columns
 constexpr int A_STAGE_BYTES = BLOCK_M * BLOCK_K * 2;        // 16 KB
@@ -83,7 +87,7 @@ __device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterp
 
 // scd_tc_kv.cu: can the specialised paged-KV kernel take this launch?  (head_dim 128, HALF RoPE,
 // 256-column tiles, whole tiles only.)  P.M/N/K/block_n/split/rope fields must be filled.
-bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P);
+bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P, long long pool_slots);
 scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s);
 
 }  // namespace scd

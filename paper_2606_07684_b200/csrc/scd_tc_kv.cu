@@ -18,6 +18,10 @@
 
 #include "scd_tc_common.cuh"
 
+#ifndef KV_STATIC_PCT
+#define KV_STATIC_PCT 60
+#endif
+
 namespace scd {
 
 namespace {
@@ -31,8 +35,11 @@ constexpr int KV_VEC_BYTES = KV_EPI_WARPS * 64 * 4;          // per-warp slice o
 struct __align__(8) KvBarriers {
   uint64_t full[MAX_STAGES], empty[MAX_STAGES];
   uint64_t tmem_full[2], tmem_empty[2];
+  uint64_t sched_full[4], sched_empty[4];                    // chunk ring (KV_SCHED_SLOTS)
+  int32_t sched_begin[4], sched_end[4];                      // tile range of the entry; begin < 0 = no more work
   uint32_t tmem_base;
 };
+constexpr int KV_SCHED_SLOTS = 4;
 
 size_t kv_smem_bytes(int stages) {
   return 1024 + (size_t)stages * (A_STAGE_BYTES + KV_B_STAGE_BYTES) + KV_STG_BYTES + KV_VEC_BYTES + sizeof(KvBarriers);
@@ -54,6 +61,9 @@ __device__ __forceinline__ uint32_t qstg_addr(uint32_t stg, int row, int chunk) 
 struct TileCoord {
   int m_tile, seg, n_tile;
 };
+__device__ __forceinline__ void tile_next(const TcParams& P, TileCoord& c) {
+  if (++c.n_tile == P.n_tiles) { c.n_tile = 0; if (++c.seg == P.n_segs) { c.seg = 0; ++c.m_tile; } }
+}
 __device__ __forceinline__ TileCoord tile_coord(const TcParams& P, int tile) {
   const int per_m = P.n_segs * P.n_tiles;
   TileCoord c;
@@ -74,6 +84,10 @@ __device__ __forceinline__ TileCoord tile_coord(const TcParams& P, int tile) {
 constexpr int KV_FIRST_EPI_WARP = 4;
 constexpr int KV_NTHREADS = (KV_FIRST_EPI_WARP + KV_EPI_WARPS) * 32;   // 640
 
+// DYN: dynamic tile scheduling (hybrid static share + claimed chunks) -- used where tiles are long (PATCH GEMM-3,
+// K = d_model) and SMs drift apart; the REUSE decode keeps the static split, whose epilogue has no registers
+// to spare for the scheduler state.
+template <bool DYN>
 __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -86,8 +100,9 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.m_tiles * P.n_segs * P.n_tiles;
-  const int t_begin = (int)((long long)total_tiles * blockIdx.x / gridDim.x);
-  const int t_end = (int)((long long)total_tiles * (blockIdx.x + 1) / gridDim.x);
+  // static mode: one contiguous share per CTA
+  const int s_begin = (int)((long long)total_tiles * blockIdx.x / gridDim.x);
+  const int s_end = (int)((long long)total_tiles * (blockIdx.x + 1) / gridDim.x);
 
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
@@ -97,6 +112,10 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
       ptx::mbar_init(&bars->tmem_empty[a], 4);          // one arrival per lane quadrant
+    }
+    for (int a = 0; a < KV_SCHED_SLOTS; ++a) {
+      ptx::mbar_init(&bars->sched_full[a], 1);
+      ptx::mbar_init(&bars->sched_empty[a], 1 + KV_EPI_WARPS);   // MMA thread + one lane per epilogue warp
     }
     ptx::fence_barrier_init();
   }
@@ -116,8 +135,36 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int tile = t_begin; tile < t_end; ++tile) {
-        const TileCoord tc = tile_coord(P, tile);
+      int slot = 0;
+      uint32_t sphase = 0;
+      // dynamic mode: every CTA owns a static contiguous share first (per-row state is computed once per m-tile), then
+      // claims small chunks of the remainder; the next claim is always in flight under the current loads
+      int next_chunk = DYN ? atomicAdd(P.sched, 1) : 0;
+      for (int round = 0;; ++round) {
+        int t_begin, t_end;
+        if (!DYN) {
+          if (round) break;
+          t_begin = s_begin;
+          t_end = s_end;
+        } else {
+        if (round == 0) {
+          t_begin = (int)blockIdx.x * P.static_tiles;
+          t_end = t_begin + P.static_tiles;
+        } else {
+          const int chunk = next_chunk;
+          if (chunk < P.n_chunks) next_chunk = atomicAdd(P.sched, 1);
+          t_begin = chunk < P.n_chunks ? P.dyn_begin + chunk * P.chunk_tiles : -1;
+          t_end = t_begin + P.chunk_tiles;
+        }
+        ptx::mbar_wait_suspend(&bars->sched_empty[slot], sphase ^ 1);
+        *(volatile int*)&bars->sched_begin[slot] = t_begin;
+        *(volatile int*)&bars->sched_end[slot] = t_end;
+        ptx::mbar_arrive(&bars->sched_full[slot]);
+        if (++slot == KV_SCHED_SLOTS) { slot = 0; sphase ^= 1; }
+        if (t_begin < 0) break;
+        }
+      TileCoord tc = tile_coord(P, t_begin);
+      for (int tile = t_begin; tile < t_end; ++tile, tile_next(P, tc)) {
         const TcSeg& sg = P.segs[tc.seg];
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
@@ -131,6 +178,16 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
+      }
+      if (DYN) {
+        // the last CTA to stop claiming work re-arms the counters for the next launch
+        __threadfence();
+        if (atomicAdd(P.sched + 1, 1) == (int)gridDim.x - 1) {
+          P.sched[0] = 0;
+          P.sched[1] = 0;
+          __threadfence();
+        }
+      }
     }
   } else if (warp == 1) {
     // ============================== MMA issuer ==============================
@@ -139,6 +196,20 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
+      int slot = 0;
+      uint32_t sphase = 0;
+      for (int round = 0;; ++round) {
+        int t_begin = s_begin, t_end = s_end;
+        if (!DYN) {
+          if (round) break;
+        } else {
+          ptx::mbar_wait_suspend(&bars->sched_full[slot], sphase);
+          t_begin = *(volatile int*)&bars->sched_begin[slot];
+          t_end = *(volatile int*)&bars->sched_end[slot];
+          ptx::mbar_arrive(&bars->sched_empty[slot]);
+          if (++slot == KV_SCHED_SLOTS) { slot = 0; sphase ^= 1; }
+          if (t_begin < 0) break;
+        }
       for (int tile = t_begin; tile < t_end; ++tile, ++it) {
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
@@ -157,6 +228,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
         ptx::mma_commit(&bars->tmem_full[acc]);
+      }
       }
     }
   }
@@ -183,11 +255,10 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       float4 vec;
       float a_scale;
     };
-    auto fetch = [&](int tile) -> Pre {
+    auto fetch = [&](const TileCoord& tc) -> Pre {
       Pre pr;
       pr.vec = make_float4(0.f, 0.f, 0.f, 0.f);
       pr.a_scale = 1.0f;
-      const TileCoord tc = tile_coord(P, tile);
       const TcSeg& sg = P.segs[tc.seg];
       const int n0 = tc.n_tile * KV_BLOCK_N;
       if (sg.col_vec && lane < 16) {
@@ -202,11 +273,28 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       return pr;
     };
 
-    Pre cur;
-    if (t_begin < t_end) cur = fetch(t_begin);
     int it = 0;
+    int sslot = 0;
+    uint32_t sphase = 0;
+    for (int round = 0;; ++round) {
+      int t_begin = s_begin, t_end = s_end;
+      if (!DYN) {
+        if (round) break;
+      } else {
+        ptx::mbar_wait_suspend(&bars->sched_full[sslot], sphase);
+        t_begin = *(volatile int*)&bars->sched_begin[sslot];
+        t_end = *(volatile int*)&bars->sched_end[sslot];
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->sched_empty[sslot]);
+        if (++sslot == KV_SCHED_SLOTS) { sslot = 0; sphase ^= 1; }
+        if (t_begin < 0) break;
+      }
+    Pre cur;
+    TileCoord tc = tile_coord(P, t_begin);
+    if (t_begin < t_end) cur = fetch(tc);
     for (int tile = t_begin; tile < t_end; ++tile, ++it) {
-      const TileCoord tc = tile_coord(P, tile);
+      TileCoord tn = tc;
+      tile_next(P, tn);
       const TcSeg& sg = P.segs[tc.seg];
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
@@ -255,7 +343,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       const uint32_t t_row = tmem_base + (uint32_t)(acc * KV_BLOCK_N) + ((uint32_t)(q * 32) << 16);
 
       Pre nxt = cur;
-      if (tile + 1 < t_end) nxt = fetch(tile + 1);
+      if (tile + 1 < t_end) nxt = fetch(tn);
 
       if (is_k) {
         // ---- K tile: rotate pairs (j, j + 64) of both heads, j in [16g, 16g + 16) ----
@@ -335,6 +423,8 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
           if (base[i] != 0ull) ptx::stg128(base[i] + (unsigned long long)lane * 16ull, v[i]);
       }
       cur = nxt;
+      tc = tn;
+    }
     }
   }
 
@@ -347,7 +437,8 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
 // ---------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------
-bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P) {
+bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P, long long pool_slots) {
+  (void)pool_slots;
   if (p->model.head_dim != 128 || p->model.rope_style != SCD_ROPE_HALF) return false;
   if (P.block_n != KV_BLOCK_N || (P.N % KV_BLOCK_N) || (P.split % KV_BLOCK_N) || P.a_kb_per_head != 0) return false;
   for (int i = 0; i < P.n_segs; ++i) {
@@ -367,13 +458,26 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   const size_t smem = kv_smem_bytes(P.stages);
   static thread_local size_t configured = 0;
   if (configured < smem) {
-    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
     configured = smem;
   }
   const int grid = std::min(total, p->sm_count);
+  // long tiles (K = d_model: PATCH GEMM-3): KV_STATIC_PCT % of an even split is owned statically, the rest is
+  // claimed tile by tile; short tiles (REUSE decode): static split only
+  const bool dyn = P.num_kb >= 16 && total > grid;
   prof_begin(s);
-  tc_kv_kernel<<<grid, KV_NTHREADS, smem, s>>>(P);
+  if (dyn) {
+    P.chunk_tiles = 1;
+    P.static_tiles = (int)((long long)total * KV_STATIC_PCT / 100 / grid);
+    P.dyn_begin = grid * P.static_tiles;
+    P.n_chunks = total - P.dyn_begin;
+    P.sched = p->kv_sched + 2 * (p->kv_sched_next.fetch_add(1) % KV_SCHED_SETS);
+    tc_kv_kernel<true><<<grid, KV_NTHREADS, smem, s>>>(P);
+  } else {
+    tc_kv_kernel<false><<<grid, KV_NTHREADS, smem, s>>>(P);
+  }
   prof_end(s, 100 + 10 * EPI_KV);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_kv_kernel launch: %s", cudaGetErrorString(e));
