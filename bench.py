@@ -257,20 +257,6 @@ def run_ours(args, cfg):
     for kid, ms in recs:
         by_kernel.setdefault(kid, []).append(ms)
 
-    # ---- write-only ceiling of this box: REUSE decode is ~90 % writes, and a plain
-    # fill sustains well below the copy figure that MEASURED_PEAKS.json reports ----
-    fill_buf = torch.empty(1 << 29, dtype=torch.bfloat16, device=dev)
-    for _ in range(3):
-        fill_buf.zero_()
-    a, b = ev(), ev()
-    a.record(stream)
-    for _ in range(10):
-        fill_buf.zero_()
-    b.record(stream)
-    torch.cuda.synchronize()
-    write_ceiling_gbs = fill_buf.numel() * 2 * 10 / (a.elapsed_time(b) * 1e-3) / 1e9
-    del fill_buf
-
     # ---- e2e: host buffers in, host buffers out ----
     e2e = None
     if not args.no_e2e:
@@ -343,8 +329,7 @@ def run_ours(args, cfg):
                                              "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                                              "traffic": traffic.get("reuse_decode"), "ms": a_ms,
                                              "share_of_step": a_ms / step_ms,
-                                             "write_gbs": wr, "write_only_ceiling_gbs": write_ceiling_gbs,
-                                             "frac_of_write_ceiling": wr / write_ceiling_gbs}
+                                             "write_gbs": wr}
             if g3_ts:
                 a_ms = sum(g3_ts) / len(g3_ts)
                 ach = costs["gemm3_flops_per_launch"] / (a_ms * 1e-3) / 1e12
@@ -386,7 +371,7 @@ def run_ours(args, cfg):
         "kv_tokens_per_s_reuse_plus_patch": tokens / ((dec_ms + pat_ms) * 1e-3),
         "kv_gbs_written": costs["kv_bytes_written"] * world / ((dec_ms + pat_ms) * 1e-3) / 1e9,
         "reuse_decode_tokens_per_s": tokens / (dec_ms * 1e-3) if dec_ms else None,
-        "gpu_launches": launches, "wall_s_timed_region": t_wall, "write_only_ceiling_gbs": write_ceiling_gbs,
+        "gpu_launches": launches, "wall_s_timed_region": t_wall,
         "clocks": clocks, "roofline": roofline, "rooflines": rooflines,
     }
     if e2e:

@@ -26,6 +26,10 @@
 
 namespace scd {
 
+// A_DEROPE: 16 extra warps rotate the K tile in shared memory, 4 threads per token row
+constexpr int DEROPE_WARPS = 16;
+constexpr int DEROPE_NTHREADS = (4 + EPI_WARPS + DEROPE_WARPS) * 32;   // 896
+
 struct __align__(8) TcBarriers {
   uint64_t full[MAX_STAGES], empty[MAX_STAGES], ready[MAX_STAGES];
   uint64_t tmem_full[2], tmem_empty[2];
@@ -156,7 +160,7 @@ __device__ __forceinline__ void rope_tile_h128_copy_out(uint32_t stg, unsigned l
 // the kernel
 // ---------------------------------------------------------------------------------
 template <int EPI, int AMODE>
-__global__ void __launch_bounds__(AMODE == A_DEROPE ? 512 : 384, 1)
+__global__ void __launch_bounds__(AMODE == A_DEROPE ? DEROPE_NTHREADS : 384, 1)
 tc_gemm_kernel(const __grid_constant__ TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -176,7 +180,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     for (int s = 0; s < STAGES; ++s) {
       ptx::mbar_init(&bars->full[s], 1);
       ptx::mbar_init(&bars->empty[s], 1);
-      ptx::mbar_init(&bars->ready[s], 128);
+      ptx::mbar_init(&bars->ready[s], DEROPE_WARPS * 32);
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
@@ -193,6 +197,10 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
 
+  // A_DEROPE: 896 threads x 72 registers, re-dealt per role: control warps 24, epilogue warps 128,
+  // rotation warps 56 (= 64512)
+  if (warp < 4) {
+  if (AMODE == A_DEROPE) ptx::setmaxnreg_dec<24>();
   if (warp == 0) {
     // ============================== TMA producer ==============================
     if (lane == 0) {
@@ -245,8 +253,10 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         ptx::mma_commit(&bars->tmem_full[acc]);
       }
     }
-  } else if (warp >= 4 && warp < 4 + EPI_WARPS) {
+  }
+  } else if (warp < 4 + EPI_WARPS) {
     // ============================== epilogue ==============================
+    if (AMODE == A_DEROPE) ptx::setmaxnreg_inc<128>();
     // One token row per thread (TMEM lane); warps w and w+4 share a lane quadrant and split the
     // tile's work into two groups (columns, or RoPE frequencies for 2-head K tiles).  Per group:
     // TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced 16-B stores.
@@ -496,15 +506,27 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = ss_u;
       cur = nxt;
     }
-  } else if (AMODE == A_DEROPE && warp >= 4 + EPI_WARPS) {
+  } else if (AMODE == A_DEROPE) {
     // ============================== A transform: deRoPE in shared memory ==============================
-    // One token row per thread.  A k-block row is 128 B = 8 chunks of 16 B, chunk c stored at
-    // position c ^ (row & 7) (128-byte swizzle).  Channel pairs (j, j + d_h/2) of a head:
+    ptx::setmaxnreg_dec<56>();
+    // Four threads per token row (the rotation, not the MMA, is what has to keep up with HBM here).  A k-block
+    // row is 128 B = 8 chunks of 16 B, chunk c stored at position c ^ (row & 7) (128-byte swizzle).  Channel
+    // pairs (j, j + d_h/2) of a head:
     //   d_h = 128: same chunk / element of two consecutive k-blocks (stages s, s+1)
     //   d_h =  64: chunks c and c + 4 of one k-block;  d_h = 32: chunks c and c + 2 (two heads per block)
-    // (cos, sin) of the row's position are computed once per tile and kept in registers.
-    const int tr = threadIdx.x - (4 + EPI_WARPS) * 32;   // 0..127 = row in tile
+    // Thread `sp` of a row owns `per` of the `pair_chunks` "a"-half chunks (8 frequencies each); its (cos, sin)
+    // of the row's position are computed once per tile and kept in registers.
+    const int dt = threadIdx.x - (4 + EPI_WARPS) * 32;
+    const int tr = dt & 127;                                            // row in tile
+    const int sp = dt >> 7;                                             // 0..3
     const int half = P.head_dim / 2;
+    const int step = P.head_dim == 128 ? 2 : 1;                         // k-blocks consumed per iteration
+    const int pair_chunks = P.head_dim == 128 ? 8 : half / 8;           // chunks in the "a" half: 8 / 4 / 2
+    const int groups = P.head_dim == 128 ? 1 : BLOCK_K / P.head_dim;    // heads per k-block
+    const int nsplit = pair_chunks < 4 ? pair_chunks : 4;
+    const int per = pair_chunks / nsplit;                               // 2 / 1 / 1
+    const bool active = sp < nsplit;
+    const uint32_t row_off = (uint32_t)(tr >> 3) * 1024 + (uint32_t)(tr & 7) * 128;
     int stage = 0;
     uint32_t phase = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
@@ -512,47 +534,47 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       const int row = m_tile * BLOCK_M + tr;
       int pos = 0;
       long long slot;
-      if (row < P.M) row_to_pos_slot(P.batch, row, pos, slot);
-      __half2 cs[64];                                   // fp16 (2^-12 abs) is below the bf16 operand rounding
+      if (row < P.M && active) row_to_pos_slot(P.batch, row, pos, slot);
+      __half2 cs[16];                                   // fp16 (2^-12 abs) is below the bf16 operand rounding
 #pragma unroll
-      for (int j = 0; j < 64; ++j) {
-        const float2 f = (j < half) ? rope_cs(pos, P.rope_g[j]) : make_float2(1.f, 0.f);
-        cs[j] = __floats2half2_rn(f.x, f.y);
+      for (int j = 0; j < 16; ++j) {
+        const int f = sp * per * 8 + j;
+        const float2 v = (active && j < per * 8) ? rope_cs(pos, P.rope_g[f & 63]) : make_float2(1.f, 0.f);
+        cs[j] = __floats2half2_rn(v.x, v.y);
       }
-      const uint32_t row_off = (uint32_t)(tr >> 3) * 1024 + (uint32_t)(tr & 7) * 128;
-      const int step = P.head_dim == 128 ? 2 : 1;     // k-blocks consumed per iteration
-      const int pair_chunks = P.head_dim == 128 ? 8 : half / 8;         // chunks in the "a" half
-      const int groups = P.head_dim == 128 ? 1 : BLOCK_K / P.head_dim;  // heads per k-block
       for (int kb = 0; kb < P.num_kb; kb += step) {
         const int s0 = stage, s1 = (stage + 1) % STAGES;
         ptx::mbar_wait_suspend(&bars->full[s0], phase);
         if (step == 2) ptx::mbar_wait_suspend(&bars->full[s1], (s1 == 0) ? (phase ^ 1) : phase);
-        uint8_t* ra = smem_a + s0 * A_STAGE_BYTES + row_off;
-        uint8_t* rb = step == 2 ? smem_a + s1 * A_STAGE_BYTES + row_off : ra;
-        for (int gidx = 0; gidx < groups; ++gidx)
+        if (active) {
+          uint8_t* ra = smem_a + s0 * A_STAGE_BYTES + row_off;
+          uint8_t* rb = step == 2 ? smem_a + s1 * A_STAGE_BYTES + row_off : ra;
+          for (int gidx = 0; gidx < groups; ++gidx)
 #pragma unroll
-          for (int cc = 0; cc < 8; ++cc) {
-            if (cc >= pair_chunks) break;
-            const int ca = P.head_dim == 128 ? cc : gidx * (P.head_dim / 8) + cc;
-            const int cb = P.head_dim == 128 ? cc : ca + pair_chunks;
-            uint4* pa = reinterpret_cast<uint4*>(ra + ((ca ^ (tr & 7)) << 4));
-            uint4* pb = reinterpret_cast<uint4*>(rb + ((cb ^ (tr & 7)) << 4));
-            uint4 xa = *pa, xb = *pb;
-            uint32_t* wa = reinterpret_cast<uint32_t*>(&xa);
-            uint32_t* wb = reinterpret_cast<uint32_t*>(&xb);
+            for (int c = 0; c < 2; ++c) {
+              if (c >= per) break;
+              const int cl = sp * per + c;                            // chunk within the "a" half
+              const int ca = P.head_dim == 128 ? cl : gidx * (P.head_dim / 8) + cl;
+              const int cb = P.head_dim == 128 ? cl : ca + pair_chunks;
+              uint4* pa = reinterpret_cast<uint4*>(ra + ((ca ^ (tr & 7)) << 4));
+              uint4* pb = reinterpret_cast<uint4*>(rb + ((cb ^ (tr & 7)) << 4));
+              uint4 xa = *pa, xb = *pb;
+              uint32_t* wa = reinterpret_cast<uint32_t*>(&xa);
+              uint32_t* wb = reinterpret_cast<uint32_t*>(&xb);
 #pragma unroll
-            for (int w = 0; w < 4; ++w) {
-              const float2 a2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wa[w]));
-              const float2 b2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wb[w]));
-              const float2 c0 = __half22float2(cs[cc * 8 + 2 * w]), c1 = __half22float2(cs[cc * 8 + 2 * w + 1]);
-              // rotation by -phi:  a' = a cos + b sin ; b' = b cos - a sin
-              wa[w] = pack_bf16x2(a2.x * c0.x + b2.x * c0.y, a2.y * c1.x + b2.y * c1.y);
-              wb[w] = pack_bf16x2(b2.x * c0.x - a2.x * c0.y, b2.y * c1.x - a2.y * c1.y);
+              for (int w = 0; w < 4; ++w) {
+                const float2 a2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wa[w]));
+                const float2 b2 = __bfloat1622float2(*reinterpret_cast<__nv_bfloat162*>(&wb[w]));
+                const float2 c0 = __half22float2(cs[c * 8 + 2 * w]), c1 = __half22float2(cs[c * 8 + 2 * w + 1]);
+                // rotation by -phi:  a' = a cos + b sin ; b' = b cos - a sin
+                wa[w] = pack_bf16x2(a2.x * c0.x + b2.x * c0.y, a2.y * c1.x + b2.y * c1.y);
+                wb[w] = pack_bf16x2(b2.x * c0.x - a2.x * c0.y, b2.y * c1.x - a2.y * c1.y);
+              }
+              *pa = xa;
+              *pb = xb;
             }
-            *pa = xa;
-            *pb = xb;
-          }
-        ptx::fence_proxy_async_smem();
+          ptx::fence_proxy_async_smem();
+        }
         ptx::mbar_arrive(&bars->ready[s0]);
         if (step == 2) ptx::mbar_arrive(&bars->ready[s1]);
         for (int q = 0; q < step; ++q)
@@ -701,7 +723,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   }
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
-  tc_gemm_kernel<EPI, AMODE><<<grid, AMODE == A_DEROPE ? 512 : 384, smem, s>>>(P);
+  tc_gemm_kernel<EPI, AMODE><<<grid, AMODE == A_DEROPE ? DEROPE_NTHREADS : 384, smem, s>>>(P);
   prof_end(s, 100 + 10 * EPI + AMODE);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));
