@@ -517,7 +517,7 @@ scd_status_t scd_reuse_decode(const scd_plan_t* plan, const scd_batch_t* batch, 
   plan_layout(plan, T, &lay);
 
   // e4m3 codes as the A operand: tensor-core expansion not built yet -> SIMT kernels
-  if (plan->use_tc && m.code_dtype != SCD_E4M3_ROWSCALE) return tc_reuse_decode(plan, batch, codes, kv, lay.off, lay.soff, (cudaStream_t)stream);
+  if (plan->use_tc) return tc_reuse_decode(plan, batch, codes, kv, lay.off, lay.soff, (cudaStream_t)stream);
 
   BatchDev bd = batch_dev(plan, batch, true);
   RopeDev rd = rope_dev(plan, false);
@@ -567,7 +567,7 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
   char* ws_u = ws_act + align_up((size_t)T * d_a_max * es, 128);
   float* ws_ss = (float*)(ws_u + align_up((size_t)T * d * es, 128));
 
-  if (plan->use_tc && m.code_dtype != SCD_E4M3_ROWSCALE)
+  if (plan->use_tc)
     return tc_patch(plan, batch, codes, kv, ws_act, ws_u, ws_ss, lay.off, lay.soff, (cudaStream_t)stream);
 
   BatchDev bd = batch_dev(plan, batch, true);

@@ -26,7 +26,8 @@
 
 namespace scd {
 
-// A_DEROPE: 16 extra warps rotate the K tile in shared memory, 4 threads per token row
+// A_DEROPE / A_CODES: 16 extra warps transform the landed A tile in shared memory, 4 threads per token row
+// (rotate the K tile by -position; expand e4m3 codes to the bf16 operand the MMA takes)
 constexpr int DEROPE_WARPS = 16;
 constexpr int DEROPE_NTHREADS = (4 + EPI_WARPS + DEROPE_WARPS) * 32;   // 896
 
@@ -49,6 +50,14 @@ static int tc_pick_stages(int block_n, int num_kb, bool even) {
   return st < 2 ? 2 : st;
 }
 
+
+// two e4m3 codes, each in the high byte of a 16-bit half -> two bf16 (exact)
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t x) {
+  const uint32_t y = (x & 0x80008000u) | ((x >> 4) & 0x07f007f0u);
+  uint32_t r;
+  asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(y), "r"(0x7b807b80u));   // x 2^120
+  return r;
+}
 
 // per-warp staging tile (shared-space address `stg`): row pitch `pitch` bytes (>= 128), 16-byte
 // chunks XOR-swizzled on the low 3 bits of the row so that row-per-thread writes and
@@ -160,7 +169,7 @@ __device__ __forceinline__ void rope_tile_h128_copy_out(uint32_t stg, unsigned l
 // the kernel
 // ---------------------------------------------------------------------------------
 template <int EPI, int AMODE>
-__global__ void __launch_bounds__(AMODE == A_DEROPE ? DEROPE_NTHREADS : 384, 1)
+__global__ void __launch_bounds__(AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, 1)
 tc_gemm_kernel(const __grid_constant__ TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -200,7 +209,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   // A_DEROPE: 896 threads x 72 registers, re-dealt per role: control warps 24, epilogue warps 128,
   // rotation warps 56 (= 64512)
   if (warp < 4) {
-  if (AMODE == A_DEROPE) ptx::setmaxnreg_dec<24>();
+  if (AMODE != A_PLAIN) ptx::setmaxnreg_dec<24>();
   if (warp == 0) {
     // ============================== TMA producer ==============================
     if (lane == 0) {
@@ -214,8 +223,12 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         const CUtensorMap* bm = P.b_maps + sg.b_map;
         for (int kb = 0; kb < P.num_kb; ++kb) {
           ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
-          ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES + b_stage_bytes);
-          if (P.a_kb_per_head > 0)
+          // A_CODES: the raw e4m3 tile [128 x 64 B] lands in the upper half of the stage and is expanded in place
+          ptx::mbar_expect_tx(&bars->full[stage], (AMODE == A_CODES ? A_STAGE_BYTES / 2 : A_STAGE_BYTES) + b_stage_bytes);
+          if (AMODE == A_CODES)
+            ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES + A_STAGE_BYTES / 2, am, &bars->full[stage], kb * BLOCK_K,
+                             m_tile * BLOCK_M, sg.a_z);
+          else if (P.a_kb_per_head > 0)
             ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES, am, &bars->full[stage],
                              (kb % P.a_kb_per_head) * BLOCK_K, kb / P.a_kb_per_head, m_tile * BLOCK_M);
           else
@@ -240,7 +253,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(acc * block_n);
         for (int kb = 0; kb < P.num_kb; ++kb) {
-          ptx::mbar_wait_suspend(AMODE == A_DEROPE ? &bars->ready[stage] : &bars->full[stage], phase);
+          ptx::mbar_wait_suspend(AMODE != A_PLAIN ? &bars->ready[stage] : &bars->full[stage], phase);
           ptx::tc_fence_after();
           const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
           const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * b_stage_bytes));
@@ -256,7 +269,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   }
   } else if (warp < 4 + EPI_WARPS) {
     // ============================== epilogue ==============================
-    if (AMODE == A_DEROPE) ptx::setmaxnreg_inc<128>();
+    if (AMODE != A_PLAIN) ptx::setmaxnreg_inc<128>();
     // One token row per thread (TMEM lane); warps w and w+4 share a lane quadrant and split the
     // tile's work into two groups (columns, or RoPE frequencies for 2-head K tiles).  Per group:
     // TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced 16-B stores.
@@ -506,6 +519,42 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = ss_u;
       cur = nxt;
     }
+  } else if (AMODE == A_CODES) {
+    // ============================== A transform: e4m3 -> bf16 in shared memory ==============================
+    // The raw tile (row-major, 64 B per token row) sits in bytes [8192, 16384) of the stage.  Thread (row, quarter)
+    // takes 16 codes, all 512 threads meet (the expansion overwrites the raw bytes), then it writes chunks
+    // 2 quarter, 2 quarter + 1 of the row in the 128-byte-swizzled K-major layout the MMA descriptor expects.
+    // e4m3 s.eeee.mmm -> bf16 s.0000eeee.mmm0000 is the same number times 2^-120 (normals and subnormals alike);
+    // one exact bf16 multiply by 2^120 finishes the conversion.  The row scale is applied in the epilogue.
+    ptx::setmaxnreg_dec<56>();
+    const int dt = threadIdx.x - (4 + EPI_WARPS) * 32;
+    const int row = dt >> 2, qt = dt & 3;
+    const uint32_t src_off = A_STAGE_BYTES / 2 + (uint32_t)dt * 16;
+    const uint32_t row_off = (uint32_t)(row >> 3) * 1024 + (uint32_t)(row & 7) * 128;
+    const uint32_t dst0 = row_off + (uint32_t)(((2 * qt) ^ (row & 7)) << 4), dst1 = row_off + (uint32_t)(((2 * qt + 1) ^ (row & 7)) << 4);
+    const uint32_t a_base = ptx::smem_u32(smem_a);
+    int stage = 0;
+    uint32_t phase = 0;
+    for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+      for (int kb = 0; kb < P.num_kb; ++kb) {
+        ptx::mbar_wait_suspend(&bars->full[stage], phase);
+        const uint32_t sb = a_base + (uint32_t)stage * A_STAGE_BYTES;
+        const uint4 raw = ptx::lds128(sb + src_off);
+        ptx::named_bar_sync(1, DEROPE_WARPS * 32);
+        const uint32_t w[4] = {raw.x, raw.y, raw.z, raw.w};
+        uint32_t o[8];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          o[2 * i] = e4m3x2_to_bf16x2(__byte_perm(w[i], 0u, 0x1404));       // bytes 0, 1 -> high bytes of two halves
+          o[2 * i + 1] = e4m3x2_to_bf16x2(__byte_perm(w[i], 0u, 0x3424));   // bytes 2, 3
+        }
+        ptx::sts128(sb + dst0, make_uint4(o[0], o[1], o[2], o[3]));
+        ptx::sts128(sb + dst1, make_uint4(o[4], o[5], o[6], o[7]));
+        ptx::fence_proxy_async_smem();
+        ptx::mbar_arrive(&bars->ready[stage]);
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+      }
+    }
   } else if (AMODE == A_DEROPE) {
     // ============================== A transform: deRoPE in shared memory ==============================
     ptx::setmaxnreg_dec<56>();
@@ -627,6 +676,24 @@ static scd_status_t make_map(CUtensorMap* m, const void* base, uint64_t d0, uint
   return SCD_OK;
 }
 
+// e4m3 code segments [n_seg][T][r] (1 byte per code): box {64, 128, 1}, no swizzle (expanded in shared memory)
+static scd_status_t make_code_map_u8(CUtensorMap* m, const void* base, uint64_t r, uint64_t T, uint64_t n_seg,
+                                     uint64_t seg_stride) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return fail(SCD_E_CUDA, "cuTensorMapEncodeTiled entry point not found");
+  cuuint64_t dims[3] = {r, T, n_seg};
+  cuuint64_t strides[2] = {r, seg_stride};
+  cuuint32_t box[3] = {BLOCK_K, BLOCK_M, 1};
+  cuuint32_t es[3] = {1, 1, 1};
+  CUresult rc = fn(m, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void*>(base), dims, strides, box, es,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (rc != CUDA_SUCCESS)
+    return fail(SCD_E_CUDA, "cuTensorMapEncodeTiled (u8 codes %llu x %llu x %llu) failed (%d)", (unsigned long long)r,
+                (unsigned long long)T, (unsigned long long)n_seg, (int)rc);
+  return SCD_OK;
+}
+
 // Bt [N, K] K-major, 2-D
 static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, int block_n) {
   EncodeTiledFn fn = encode_fn();
@@ -713,7 +780,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.num_kb = (P.K + BLOCK_K - 1) / BLOCK_K;
   const int total = P.n_segs * P.m_tiles * P.n_tiles;
   if (total <= 0) return SCD_OK;
-  P.stages = tc_pick_stages(P.block_n, P.num_kb, AMODE == A_DEROPE);
+  P.stages = tc_pick_stages(P.block_n, P.num_kb, AMODE == A_DEROPE);   // deRoPE pairs k-blocks
   const size_t smem = tc_smem_bytes(P.block_n, P.stages);
   static thread_local size_t configured = 0;   // per instantiation
   if (configured < smem) {
@@ -723,7 +790,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   }
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
-  tc_gemm_kernel<EPI, AMODE><<<grid, AMODE == A_DEROPE ? DEROPE_NTHREADS : 384, smem, s>>>(P);
+  tc_gemm_kernel<EPI, AMODE><<<grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, smem, s>>>(P);
   prof_end(s, 100 + 10 * EPI + AMODE);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));
@@ -833,7 +900,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
                              const scd_paged_kv_t* kv, const size_t* off, const size_t* soff, cudaStream_t s) {
   const scd_model_desc_t& m = p->model;
   const int T = batch->total_tokens;
-  if (m.code_dtype == SCD_E4M3_ROWSCALE) return fail(SCD_E_UNSUPPORTED, "e4m3 decode on tensor cores: not yet");
+  const bool e4 = m.code_dtype == SCD_E4M3_ROWSCALE;
   scd_status_t st;
   const int nseg_all = (int)p->segs.size();
   size_t i = 0;
@@ -853,7 +920,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
     P.split = P.N;
     P.pool_width = p->D;
     // segments of a run are consecutive in the code buffer with a uniform stride: one 3-D map
-    const size_t seg_stride = align_up((size_t)T * s0.rank * 2, 128);
+    const size_t seg_stride = align_up((size_t)T * s0.rank * (e4 ? 1 : 2), 128);
     const int key0 = s0.layer * 3 + s0.branch;
     bool uniform = true;
     for (size_t q = i; q < j; ++q) {
@@ -861,9 +928,10 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
       if (off[sp.layer * 3 + sp.branch] != off[key0] + (q - i) * seg_stride) uniform = false;
     }
     if (uniform) {
-      if ((st = make_map(&P.a_maps[0], (const char*)codes + off[key0], s0.rank, T, j - i, (uint64_t)s0.rank * 2,
-                         seg_stride, BLOCK_M, 1)) != SCD_OK)
-        return st;
+      st = e4 ? make_code_map_u8(&P.a_maps[0], (const char*)codes + off[key0], s0.rank, T, j - i, seg_stride)
+              : make_map(&P.a_maps[0], (const char*)codes + off[key0], s0.rank, T, j - i, (uint64_t)s0.rank * 2, seg_stride,
+                         BLOCK_M, 1);
+      if (st != SCD_OK) return st;
     }
     for (size_t q = i; q < j; ++q) {
       const SegPlan& sp = p->segs[reuse[q]];
@@ -873,21 +941,24 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
       sg.out0 = sp.branch == SCD_BRANCH_K ? kv->k_pool[sp.layer] : kv->v_pool[sp.layer];
       sg.rope_cols = (sp.branch == SCD_BRANCH_K && m.rope_on_reuse_k) ? p->D : 0;
       sg.b_map = nseg_all + sp.seg_index;
+      sg.a_scale = e4 ? (const float*)((const char*)codes + soff[key]) : nullptr;
       if (uniform) {
         sg.a_map = 0;
         sg.a_z = (int)(q - i);
       } else {
         sg.a_map = (int)(q - i);
         sg.a_z = 0;
-        if ((st = make_map(&P.a_maps[q - i], (const char*)codes + off[key], sp.rank, T, 1, (uint64_t)sp.rank * 2,
-                           seg_stride, BLOCK_M, 1)) != SCD_OK)
-          return st;
+        st = e4 ? make_code_map_u8(&P.a_maps[q - i], (const char*)codes + off[key], sp.rank, T, 1, seg_stride)
+                : make_map(&P.a_maps[q - i], (const char*)codes + off[key], sp.rank, T, 1, (uint64_t)sp.rank * 2, seg_stride,
+                           BLOCK_M, 1);
+        if (st != SCD_OK) return st;
       }
     }
-    if ((st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
+    if (e4) st = launch_tc<EPI_KV, A_CODES>(p, P, s);       // operand expansion in shared memory (generic kernel)
+    else st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
+    if (st != SCD_OK) return st;
     i = j;
   }
-  (void)soff;
   return SCD_OK;
 }
 
@@ -899,7 +970,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
                       void* ws_act, void* ws_u, float* ws_ss, const size_t* off, const size_t* soff, cudaStream_t s) {
   const scd_model_desc_t& m = p->model;
   const int T = batch->total_tokens, d = m.d_model, D = p->D;
-  if (m.code_dtype == SCD_E4M3_ROWSCALE) return fail(SCD_E_UNSUPPORTED, "e4m3 patch on tensor cores: not yet");
+  const bool e4 = m.code_dtype == SCD_E4M3_ROWSCALE;
   const bool rms = m.patch_norm == SCD_NORM_RMS;
   const int nseg = (int)p->segs.size();
   scd_status_t st;
@@ -910,10 +981,13 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     // GEMM-1: [T, r_h] x [r_h, d_a]
     fill_common(p, batch, true, false, P);
     P.n_segs = 1; P.N = pp.d_a; P.K = pp.r_h; P.block_n = pick_block_n_cover(pp.d_a);
-    if ((st = make_map(&P.a_maps[0], (const char*)codes + off[key], pp.r_h, T, 1, (uint64_t)pp.r_h * 2,
-                       align_up((size_t)T * pp.r_h * 2, 128), BLOCK_M, 1)) != SCD_OK) return st;
+    st = e4 ? make_code_map_u8(&P.a_maps[0], (const char*)codes + off[key], pp.r_h, T, 1, align_up((size_t)T * pp.r_h, 128))
+            : make_map(&P.a_maps[0], (const char*)codes + off[key], pp.r_h, T, 1, (uint64_t)pp.r_h * 2,
+                       align_up((size_t)T * pp.r_h * 2, 128), BLOCK_M, 1);
+    if (st != SCD_OK) return st;
     P.segs[0].col_vec = pp.b1; P.segs[0].out0 = ws_act; P.segs[0].b_map = 2 * nseg + 3 * (int)j;
-    if ((st = launch_tc<EPI_ACT, A_PLAIN>(p, P, s)) != SCD_OK) return st;
+    P.segs[0].a_scale = e4 ? (const float*)((const char*)codes + soff[key]) : nullptr;
+    if ((st = e4 ? launch_tc<EPI_ACT, A_CODES>(p, P, s) : launch_tc<EPI_ACT, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     // GEMM-2: [T, d_a] x [d_a, d]
     fill_common(p, batch, true, false, P);
     P.n_segs = 1; P.N = d; P.K = pp.d_a; P.block_n = pick_block_n_cover(d);
@@ -932,7 +1006,6 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     P.segs[0].b_map = 2 * nseg + 3 * (int)j + 2;
     if ((st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
   }
-  (void)soff;
   return SCD_OK;
 }
 

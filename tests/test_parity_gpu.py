@@ -88,6 +88,46 @@ def test_tiny_round_trip_matches_truncation_closed_form(cuda_device):
             assert 0.05 < got / np.linalg.norm(x - P.np64(mu)[None, :]) < 0.10
 
 
+def test_e4m3_operand_expansion_is_exact_for_every_code(cuda_device):
+    """The tcgen05 path widens e4m3 codes to bf16 in shared memory; that must be exact for all 254 finite
+    codes, subnormals included (a flush-to-zero would wipe rows made of small codes only).  Hand-written
+    code bytes and power-of-two scales go through scd_reuse_decode; each output element must agree with
+    the oracle (same code bits) to bf16 output rounding."""
+    cfg = MINI["mistral_7b_32k_fp8"].scaled(n_layers=1, patch_layers=(), seqlens=(256,))
+    prob = _problem(cfg, cuda_device, use_means=False)
+    prob.alloc_pools()
+    finite = np.array([b for b in range(256) if (b & 0x7F) != 0x7F], dtype=np.uint8)
+    small = np.array([b for b in range(256) if (b & 0x78) == 0], dtype=np.uint8)       # zero + subnormals, both signs
+    rng = np.random.default_rng(0)
+    for br in (O.BRANCH_K, O.BRANCH_V):
+        q, s = prob.code_view(0, br)
+        T, r = q.shape
+        codes = np.empty((T, r), np.uint8)
+        for t in range(T):
+            pool = small if t % 4 == 3 else finite            # every 4th row: small codes only
+            codes[t] = np.roll(np.resize(pool, r), t)
+        q.copy_(torch.from_numpy(codes).to(cuda_device))
+        s.copy_(torch.from_numpy((2.0 ** rng.integers(-6, 3, T)).astype(np.float32)).to(cuda_device))
+    prob.reuse_decode()
+    torch.cuda.synchronize()
+    om, ob = P.oracle_model(prob), P.oracle_batch(prob)
+    pos, slots = O.positions(ob), O.slot_mapping(ob, om.block_size)
+    ol = P.oracle_layer(prob, 0)
+    qk, sk = P.gpu_codes(prob, 0, O.BRANCH_K)
+    qv, sv = P.gpu_codes(prob, 0, O.BRANCH_V)
+    zk, zv = O.unpack_codes(qk, sk, om.code_dtype), O.unpack_codes(qv, sv, om.code_dtype)
+    k_o, v_o = O.reuse_decode_layer(om, ol, zk, zv, pos)
+    for name, z, dec, want, pool in (("K", zk, ol.dec_k, k_o, prob.k_pool[0]), ("V", zv, ol.dec_v, v_o, prob.v_pool[0])):
+        got = P._gather(pool, slots)
+        # bf16 output rounding (2^-9 relative) + fp32 accumulation of r products (and the RoPE mix for K)
+        bound = 2.0 ** -8 * np.abs(want) + 1e-5 * (np.abs(z) @ np.abs(dec)) + 1e-30
+        if name == "K":
+            bound = bound + 2.0 ** -8 * np.sqrt((want.reshape(len(want), -1, cfg.head_dim) ** 2).sum(-1)).repeat(cfg.head_dim, axis=1)
+        bad = np.abs(got - want) > bound
+        assert not bad.any(), f"{name}: {int(bad.sum())} elements off, first at {np.argwhere(bad)[0]}"
+        assert np.abs(want[3::4]).max() > 0          # the small-code rows are not trivially zero
+
+
 @pytest.mark.parametrize("state", ["f32", "bf16"])
 def test_edge_batches(state, cuda_device):
     """Ragged lengths that are not multiples of 16 / 128, a 1-token request, position offsets,
