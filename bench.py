@@ -32,8 +32,8 @@ if ROOT not in sys.path:
 METRIC = "reconstructed KV tokens/s (REUSE+PATCH hybrid cache, encode->reuse_decode->patch)"
 UNIT = "tokens/s"
 KERNEL_NAMES = {100: "tc_gemm<codes,plain> (encode V/H)", 101: "tc_gemm<codes,derope> (encode K)",
-                110: "tc_gemm<paged_kv> (reuse decode / patch GEMM-3)", 120: "tc_gemm<aligner_in> (patch GEMM-1)",
-                130: "tc_gemm<aligner_out> (patch GEMM-2)"}
+                110: "tc_kv_kernel / tc_gemm<paged_kv> (reuse decode)", 120: "tc_gemm<aligner_in> (patch GEMM-1)",
+                130: "tc_gemm<aligner_out> (patch GEMM-2)", 140: "tc_kv_kernel<dyn> (patch GEMM-3)"}
 
 
 # ------------------------------------------------------------------------------ helpers
@@ -316,28 +316,21 @@ def run_ours(args, cfg):
     for kid, ts in by_kernel.items():
         avg_ms = sum(ts) / len(ts)
         per_pass = len(ts) / n_prof
-        if kid == 110:      # paged-KV kernel: reuse decode launches (HBM) and patch GEMM-3 launches (tensor) differ
-            n_dec = 1 if cfg.n_layers > len(cfg.patch_layers) else 0
-            # launches arrive in call order: decode first, then one GEMM-3 per patch layer
-            dec_ts = [t for i, t in enumerate(ts) if n_dec and i % int(per_pass) == 0]
-            g3_ts = [t for i, t in enumerate(ts) if not (n_dec and i % int(per_pass) == 0)]
-            if dec_ts:
-                a_ms = sum(dec_ts) / len(dec_ts)
-                ach = costs["reuse_bytes"] / (a_ms * 1e-3) / 1e9
-                wr = costs["reuse_bytes_written"] / (a_ms * 1e-3) / 1e9
-                rooflines["reuse_decode"] = {"kernel": KERNEL_NAMES[kid], "bound": "hbm", "achieved": ach,
-                                             "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
-                                             "traffic": traffic.get("reuse_decode"), "ms": a_ms,
-                                             "share_of_step": a_ms / step_ms,
-                                             "write_gbs": wr}
-            if g3_ts:
-                a_ms = sum(g3_ts) / len(g3_ts)
-                ach = costs["gemm3_flops_per_launch"] / (a_ms * 1e-3) / 1e12
-                rooflines["patch_gemm3"] = {"kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach,
-                                            "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                                            "frac": ach / peaks["bf16_tflops_sustained"],
-                                            "traffic": traffic.get("patch_gemm3"), "ms": a_ms,
-                                            "share_of_step": a_ms * len(cfg.patch_layers) / step_ms}
+        if kid == 110:      # REUSE decode: one launch per call (per rank run), HBM-bound
+            call_ms = avg_ms * per_pass          # all decode launches of one call (one per run of equal ranks)
+            ach = costs["reuse_bytes"] / (call_ms * 1e-3) / 1e9
+            wr = costs["reuse_bytes_written"] / (call_ms * 1e-3) / 1e9
+            rooflines["reuse_decode"] = {"kernel": KERNEL_NAMES[kid], "bound": "hbm", "achieved": ach,
+                                         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
+                                         "traffic": traffic.get("reuse_decode"), "ms": call_ms,
+                                         "share_of_step": call_ms / step_ms, "write_gbs": wr}
+        elif kid == 140:    # PATCH GEMM-3 (+ row scale, RoPE, paged write): tensor-bound
+            ach = costs["gemm3_flops_per_launch"] / (avg_ms * 1e-3) / 1e12
+            rooflines["patch_gemm3"] = {"kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach,
+                                        "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                                        "frac": ach / peaks["bf16_tflops_sustained"],
+                                        "traffic": traffic.get("patch_gemm3"), "ms": avg_ms,
+                                        "share_of_step": avg_ms * len(cfg.patch_layers) / step_ms}
         elif kid in (120, 130):
             fl = costs["gemm1_flops_per_launch"] if kid == 120 else costs["gemm2_flops_per_launch"]
             ach = fl / (avg_ms * 1e-3) / 1e12
@@ -397,9 +390,12 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=4096)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--rank", type=int, default=0, help="override the config's rank (config 5 rank sweep)")
     args = ap.parse_args()
     from paper_2606_07684_b200 import workloads as W
     cfg = W.CONFIGS[args.config]
+    if args.rank:
+        cfg = cfg.scaled(rank=args.rank)
     if args.impl == "reference":
         run_reference(args, cfg)
         return

@@ -26,6 +26,12 @@ enum EpiKind : int {
   EPI_U = 3        // patch GEMM-2: y = acc + b2[n]; partial sum of squares per (n-tile, row)
 };
 
+// ids under which scd_profile_fetch reports the launches of the tensor-core path
+enum ProfId : int {
+  SCD_PROF_ENCODE = 100, SCD_PROF_ENCODE_K = 101, SCD_PROF_REUSE_DECODE = 110, SCD_PROF_PATCH_GEMM1 = 120,
+  SCD_PROF_PATCH_GEMM2 = 130, SCD_PROF_PATCH_GEMM3 = 140
+};
+
 enum AMode : int {
   A_PLAIN = 0,     // A is state dtype, used as is
   A_DEROPE = 1,    // A is the producer's post-RoPE K: rotate by -pos on load (Eq. 5)

@@ -51,6 +51,27 @@ static int tc_pick_stages(int block_n, int num_kb, bool even) {
 }
 
 
+// Tile order inside a segment: super-blocks of P.msb m-tiles; inside a super-block all its m-tiles for
+// n-tile 0, then n-tile 1, ...  The A rows of a super-block (msb x 128 tokens) stay L2-resident while every
+// B slice passes once per super-block, instead of A being re-streamed from HBM once per n-tile when
+// T x K x 2 B outgrows the L2 (PATCH GEMM-2 at 32k tokens: 268-537 MB).  msb >= m_tiles: plain m-fastest order.
+__device__ __forceinline__ void tile_decode(const TcParams& P, int tile, int& m_tile, int& n_tile, int& seg) {
+  const int per_seg = P.m_tiles * P.n_tiles;
+  seg = tile / per_seg;
+  const int t = tile - seg * per_seg;
+  if (P.msb >= P.m_tiles) {
+    n_tile = t / P.m_tiles;
+    m_tile = t - n_tile * P.m_tiles;
+    return;
+  }
+  const int per_sb = P.msb * P.n_tiles;
+  const int sb = t / per_sb;
+  const int rem = t - sb * per_sb;
+  const int rows = min(P.msb, P.m_tiles - sb * P.msb);     // the last super-block may be short
+  n_tile = rem / rows;
+  m_tile = sb * P.msb + (rem - n_tile * rows);
+}
+
 // two e4m3 codes, each in the high byte of a 16-bit half -> two bf16 (exact)
 __device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t x) {
   const uint32_t y = (x & 0x80008000u) | ((x >> 4) & 0x07f007f0u);
@@ -216,9 +237,9 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       int stage = 0;
       uint32_t phase = 0;
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        const int m_tile = tile % P.m_tiles;
-        const int n_tile = (tile / P.m_tiles) % P.n_tiles;
-        const TcSeg& sg = P.segs[tile / (P.m_tiles * P.n_tiles)];
+        int m_tile, n_tile, seg_i;
+        tile_decode(P, tile, m_tile, n_tile, seg_i);
+        const TcSeg& sg = P.segs[seg_i];
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
         for (int kb = 0; kb < P.num_kb; ++kb) {
@@ -296,9 +317,9 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       RowInfo ri;
       ri.pos = 0; ri.rs = 1.0f; ri.row_ptr = 0ull;
       ri.m0 = make_float4(0.f, 0.f, 0.f, 0.f); ri.m1 = ri.m0;
-      const int m_tile = tile % P.m_tiles;
-      const int n_tile = (tile / P.m_tiles) % P.n_tiles;
-      const TcSeg& sg = P.segs[tile / (P.m_tiles * P.n_tiles)];
+      int m_tile, n_tile, seg_i;
+      tile_decode(P, tile, m_tile, n_tile, seg_i);
+      const TcSeg& sg = P.segs[seg_i];
       const int row = m_tile * BLOCK_M + ew * 32 + lane;
       const int n0 = n_tile * block_n;
       if (sg.col_vec) {
@@ -329,9 +350,9 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     RowInfo cur;
     if ((int)blockIdx.x < total_tiles) cur = fetch(blockIdx.x);
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
-      const int m_tile = tile % P.m_tiles;
-      const int n_tile = (tile / P.m_tiles) % P.n_tiles;
-      const TcSeg& sg = P.segs[tile / (P.m_tiles * P.n_tiles)];
+      int m_tile, n_tile, seg_i;
+      tile_decode(P, tile, m_tile, n_tile, seg_i);
+      const TcSeg& sg = P.segs[seg_i];
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
       const int row = m_tile * BLOCK_M + ew * 32 + lane;
@@ -579,7 +600,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     int stage = 0;
     uint32_t phase = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-      const int m_tile = tile % P.m_tiles;
+      int m_tile, n_tile_unused, seg_unused;
+      tile_decode(P, tile, m_tile, n_tile_unused, seg_unused);
       const int row = m_tile * BLOCK_M + tr;
       int pos = 0;
       long long slot;
@@ -781,6 +803,13 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   const int total = P.n_segs * P.m_tiles * P.n_tiles;
   if (total <= 0) return SCD_OK;
   P.stages = tc_pick_stages(P.block_n, P.num_kb, AMODE == A_DEROPE);   // deRoPE pairs k-blocks
+  // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
+  P.msb = P.m_tiles;
+  if (P.n_tiles > 1) {
+    const long long a_tile_bytes = (long long)BLOCK_M * P.K * 2;
+    int msb = (int)std::max<long long>(1, (32ll << 20) / a_tile_bytes);
+    if (msb < P.m_tiles) P.msb = msb;
+  }
   const size_t smem = tc_smem_bytes(P.block_n, P.stages);
   static thread_local size_t configured = 0;   // per instantiation
   if (configured < smem) {
@@ -791,7 +820,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
   tc_gemm_kernel<EPI, AMODE><<<grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, smem, s>>>(P);
-  prof_end(s, 100 + 10 * EPI + AMODE);
+  prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));
   count_launch();
@@ -880,6 +909,7 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
       }
       if (st != SCD_OK) return st;
     }
+    P.prof_id = (s0.branch == SCD_BRANCH_K && m.k_is_roped) ? SCD_PROF_ENCODE_K : SCD_PROF_ENCODE;
     if (s0.branch == SCD_BRANCH_K && m.k_is_roped) {
       if (m.rope_style != SCD_ROPE_HALF)
         return fail(SCD_E_UNSUPPORTED, "deRoPE-on-load implements the HALF pairing only on the bf16 path");
@@ -954,6 +984,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
         if (st != SCD_OK) return st;
       }
     }
+    P.prof_id = SCD_PROF_REUSE_DECODE;
     if (e4) st = launch_tc<EPI_KV, A_CODES>(p, P, s);       // operand expansion in shared memory (generic kernel)
     else st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
     if (st != SCD_OK) return st;
@@ -987,6 +1018,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     if (st != SCD_OK) return st;
     P.segs[0].col_vec = pp.b1; P.segs[0].out0 = ws_act; P.segs[0].b_map = 2 * nseg + 3 * (int)j;
     P.segs[0].a_scale = e4 ? (const float*)((const char*)codes + soff[key]) : nullptr;
+    P.prof_id = SCD_PROF_PATCH_GEMM1;
     if ((st = e4 ? launch_tc<EPI_ACT, A_CODES>(p, P, s) : launch_tc<EPI_ACT, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     // GEMM-2: [T, d_a] x [d_a, d]
     fill_common(p, batch, true, false, P);
@@ -995,6 +1027,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     P.segs[0].col_vec = pp.b2; P.segs[0].out0 = ws_u; P.segs[0].aux = rms ? ws_ss : nullptr;
     P.segs[0].b_map = 2 * nseg + 3 * (int)j + 1;
     const int n_partials = 2 * ((d + P.block_n - 1) / P.block_n);   // two column groups per n-tile
+    P.prof_id = SCD_PROF_PATCH_GEMM2;
     if ((st = launch_tc<EPI_U, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     // GEMM-3: [T, d] x [d, 2D]
     fill_common(p, batch, true, false, P);
@@ -1004,6 +1037,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     P.segs[0].col_vec = pp.bkv; P.segs[0].out0 = kv->k_pool[pp.layer]; P.segs[0].out1 = kv->v_pool[pp.layer];
     P.segs[0].rowscale_in = rms ? ws_ss : nullptr; P.segs[0].rope_cols = D;
     P.segs[0].b_map = 2 * nseg + 3 * (int)j + 2;
+    P.prof_id = SCD_PROF_PATCH_GEMM3;
     if ((st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
   }
   return SCD_OK;

@@ -31,12 +31,14 @@ struct TcParams {
   BatchDev batch;
   int32_t n_segs, M, N, K;
   int32_t m_tiles, n_tiles, num_kb, block_n, stages;
+  int32_t msb;                        // generic kernel: m-tiles per L2 super-block (tile_decode)
   int32_t a_kb_per_head;              // >0: A is [T, H, d_h] head-strided, k-blocks per head
   int32_t split, pool_width, head_dim, rope_style, act, code_dtype;
   int32_t n_partials, rms_dim;
   float rms_eps;
   int32_t* sched;                     // paged-KV kernel: {next chunk, CTAs done}
   int32_t chunk_tiles, n_chunks;      // paged-KV kernel: consecutive tiles per dynamically claimed unit
+  int32_t prof_id;                    // host only: id under which scd_profile_* reports the launch
   int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
 };
 

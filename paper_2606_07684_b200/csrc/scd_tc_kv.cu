@@ -478,7 +478,7 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   } else {
     tc_kv_kernel<false><<<grid, KV_NTHREADS, smem, s>>>(P);
   }
-  prof_end(s, 100 + 10 * EPI_KV);
+  prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_kv_kernel launch: %s", cudaGetErrorString(e));
   count_launch();

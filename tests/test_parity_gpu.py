@@ -204,7 +204,7 @@ FULL_SAMPLE = {"llama3_8b_8k": 384, "llama3_8b_ragged": 256, "mistral_7b_32k_fp8
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("name", ["llama3_8b_8k", "llama3_8b_ragged", "mistral_7b_32k_fp8"])
+@pytest.mark.parametrize("name", ["llama3_8b_8k", "llama3_8b_ragged", "mistral_7b_32k_fp8", "llama3_70b_2x16k"])
 def test_full_size_sampled_parity(name, cuda_device):
     """BASELINE.json's full sizes in the launch configuration bench.py times; the oracle
     recomputes a row sample (first / last rows of every request, ragged tails, seeded random
