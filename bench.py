@@ -317,7 +317,9 @@ def run_ours(args, cfg):
         avg_ms = sum(ts) / len(ts)
         per_pass = len(ts) / n_prof
         if kid == 110:      # REUSE decode: one launch per call (per rank run), HBM-bound
-            call_ms = avg_ms * per_pass          # all decode launches of one call (one per run of equal ranks)
+            # one launch per call (all REUSE segments of equal rank): the call's own events in the timed region
+            # are the kernel's duration; several launches: sum of the in-library per-launch events
+            call_ms = dec_ms if per_pass == 1 else avg_ms * per_pass
             ach = costs["reuse_bytes"] / (call_ms * 1e-3) / 1e9
             wr = costs["reuse_bytes_written"] / (call_ms * 1e-3) / 1e9
             rooflines["reuse_decode"] = {"kernel": KERNEL_NAMES[kid], "bound": "hbm", "achieved": ach,
