@@ -60,6 +60,10 @@ class Model:
     patch_act: int = ACT_SILU
     patch_norm: int = NORM_RMS
     rms_eps: float = 1e-5
+    # Paper-literal REUSE translator: batch x heads x tokens are flattened into
+    # one sample axis and ONE map W_enc in R^{d_h x r} / W_dec in R^{r x d_h} serves every head of the layer.
+    # Codes of a token are the heads' codes side by side, [H * r].  False = per-layer basis over D.
+    reuse_per_head: bool = False
 
     @property
     def D(self) -> int:
@@ -131,8 +135,9 @@ def payload_bytes(model: Model, layers: Sequence[Layer], total_tokens: int) -> i
     n = 0
     for l in layers:
         if l.kind == REUSE:
-            n += total_tokens * (l.enc_k.shape[1] * cb + sb)
-            n += total_tokens * (l.enc_v.shape[1] * cb + sb)
+            hm = model.n_kv_heads if model.reuse_per_head else 1      # per-head: r codes per head
+            n += total_tokens * (hm * l.enc_k.shape[1] * cb + sb)
+            n += total_tokens * (hm * l.enc_v.shape[1] * cb + sb)
         else:
             n += total_tokens * (l.enc_h.shape[1] * cb + sb)
     return n
@@ -285,18 +290,30 @@ def _add(x: np.ndarray, mu: Optional[np.ndarray]) -> np.ndarray:
     return x if mu is None else x + mu[None, :]
 
 
+def _translate(model: Model, x: np.ndarray, mu: Optional[np.ndarray], w: np.ndarray, mu_after: bool) -> np.ndarray:
+    """One linear REUSE map on rows of x.  Per-layer reading: x [T, in] (in = D or r).  Per-head reading
+    (model.reuse_per_head): every head of every token is a sample, w is [d_h, r] or [r, d_h], mu is [d_h];
+    the result is laid out per token again, heads side by side."""
+    if not model.reuse_per_head:
+        return _add(x @ w, mu) if mu_after else _sub(x, mu) @ w
+    t = x.shape[0]
+    xs = x.reshape(t * model.n_kv_heads, w.shape[0])
+    ys = _add(xs @ w, mu) if mu_after else _sub(xs, mu) @ w
+    return ys.reshape(t, model.n_kv_heads * w.shape[1])
+
+
 def encode_k(model: Model, layer: Layer, k_a: np.ndarray, pos: np.ndarray) -> np.ndarray:
     """Z_K = (deRoPE(K_A) - mu_src,K) W_enc,K   (Eq. 5, Eq. 8, Alg. 1 :178)."""
     k = np.asarray(k_a, dtype=np.float64)
     if model.k_is_roped:
         k = rope(k, pos, model.rope_theta_producer, -1, model.n_kv_heads, model.head_dim,
                  model.rope_style)
-    return _sub(k, layer.mean_src_k) @ layer.enc_k
+    return _translate(model, k, layer.mean_src_k, layer.enc_k, False)
 
 
 def encode_v(model: Model, layer: Layer, v_a: np.ndarray) -> np.ndarray:
     """Z_V = (V_A - mu_src,V) W_enc,V   (Eq. 8; "Values V are processed directly" :127)."""
-    return _sub(np.asarray(v_a, dtype=np.float64), layer.mean_src_v) @ layer.enc_v
+    return _translate(model, np.asarray(v_a, dtype=np.float64), layer.mean_src_v, layer.enc_v, False)
 
 
 def encode_h(model: Model, layer: Layer, h_a: np.ndarray) -> np.ndarray:
@@ -329,11 +346,11 @@ def scd_encode(model: Model, layers: Sequence[Layer], batch: Batch,
 def reuse_decode_layer(model: Model, layer: Layer, z_k: np.ndarray, z_v: np.ndarray,
                        pos: np.ndarray) -> Tuple[np.ndarray, np.ndarray]:
     """K_B = RoPE(Z_K W_dec,K + mu_dst,K);  V_B = Z_V W_dec,V + mu_dst,V."""
-    k = _add(z_k @ layer.dec_k, layer.mean_dst_k)
+    k = _translate(model, z_k, layer.mean_dst_k, layer.dec_k, True)
     if model.rope_on_reuse_k:
         k = rope(k, pos, model.rope_theta_consumer, +1, model.n_kv_heads, model.head_dim,
                  model.rope_style)
-    v = _add(z_v @ layer.dec_v, layer.mean_dst_v)
+    v = _translate(model, z_v, layer.mean_dst_v, layer.dec_v, True)
     return k, v
 
 

@@ -501,3 +501,52 @@ def test_whole_call_tiny_against_torch_fp64():
     for i in range(3):
         np.testing.assert_array_equal(kp2[i].reshape(-1, D)[s_np[sel]], kp[i].reshape(-1, D)[s_np[sel]])
         assert np.isnan(kp2[i].reshape(-1, D)[np.setdiff1d(np.arange(80), s_np[sel])]).all()
+
+
+def test_per_head_mode_against_block_diagonal_and_scalar_loops():
+    """Paper-literal REUSE (heads flattened into the sample axis, one d_h x r map for
+    all heads) as Model(reuse_per_head=True): pinned (i) against the per-layer functions with I_H (x) W and the
+    mean tiled over heads -- the reading pinned above, now the other way round -- and (ii) against plain scalar
+    loops over (token, head, code) with RoPE from the complex-multiplication form."""
+    rng = np.random.default_rng(11)
+    T, H, d_h, r_k, r_v = 5, 3, 8, 4, 2
+    D = H * d_h
+    K, V = rng.standard_normal((T, D)), rng.standard_normal((T, D))
+    ek, dk = rng.standard_normal((d_h, r_k)), rng.standard_normal((r_k, d_h))
+    ev, dv = rng.standard_normal((d_h, r_v)), rng.standard_normal((r_v, d_h))
+    mk, mv, nk, nv = (rng.standard_normal(d_h) for _ in range(4))
+    pos = np.array([0, 3, 7, 8, 100])
+    ph = O.Model(1, 16, H, d_h, rope_theta_producer=1e4, rope_theta_consumer=5e5, reuse_per_head=True)
+    pl = O.Model(1, 16, H, d_h, rope_theta_producer=1e4, rope_theta_consumer=5e5)
+    lay_h = O.Layer(O.REUSE, enc_k=ek, dec_k=dk, enc_v=ev, dec_v=dv, mean_src_k=mk, mean_src_v=mv, mean_dst_k=nk, mean_dst_v=nv)
+    eye = np.eye(H)
+    lay_l = O.Layer(O.REUSE, enc_k=np.kron(eye, ek), dec_k=np.kron(eye, dk), enc_v=np.kron(eye, ev), dec_v=np.kron(eye, dv),
+                    mean_src_k=np.tile(mk, H), mean_src_v=np.tile(mv, H), mean_dst_k=np.tile(nk, H), mean_dst_v=np.tile(nv, H))
+    zk, zv = O.encode_k(ph, lay_h, K, pos), O.encode_v(ph, lay_h, V)
+    assert zk.shape == (T, H * r_k) and zv.shape == (T, H * r_v)
+    np.testing.assert_allclose(zk, O.encode_k(pl, lay_l, K, pos), atol=1e-12)
+    np.testing.assert_allclose(zv, O.encode_v(pl, lay_l, V), atol=1e-12)
+    k1, v1 = O.reuse_decode_layer(ph, lay_h, zk, zv, pos)
+    k2, v2 = O.reuse_decode_layer(pl, lay_l, zk, zv, pos)
+    np.testing.assert_allclose(k1, k2, atol=1e-12)
+    np.testing.assert_allclose(v1, v2, atol=1e-12)
+    # (ii) scalar loops
+    def rot(x, p, theta, sign):          # one head, HALF pairing, complex multiplication
+        out = np.empty(d_h)
+        for j in range(d_h // 2):
+            z = complex(x[j], x[j + d_h // 2]) * cmath.exp(1j * sign * p * theta ** (-2.0 * j / d_h))
+            out[j], out[j + d_h // 2] = z.real, z.imag
+        return out
+    for t in range(T):
+        for h in range(H):
+            kc = rot(K[t, h * d_h:(h + 1) * d_h], pos[t], 1e4, -1)
+            for i in range(r_k):
+                assert abs(zk[t, h * r_k + i] - sum((kc[j] - mk[j]) * ek[j, i] for j in range(d_h))) < 1e-12
+            for i in range(r_v):
+                assert abs(zv[t, h * r_v + i] - sum((V[t, h * d_h + j] - mv[j]) * ev[j, i] for j in range(d_h))) < 1e-12
+            kd = np.array([sum(zk[t, h * r_k + i] * dk[i, j] for i in range(r_k)) + nk[j] for j in range(d_h)])
+            np.testing.assert_allclose(k1[t, h * d_h:(h + 1) * d_h], rot(kd, pos[t], 5e5, +1), atol=1e-12)
+            for j in range(d_h):
+                assert abs(v1[t, h * d_h + j] - (sum(zv[t, h * r_v + i] * dv[i, j] for i in range(r_v)) + nv[j])) < 1e-12
+    # payload: H * r codes per token and branch
+    assert O.payload_bytes(ph, [lay_h], 10) == 10 * H * (r_k + r_v) * 4
