@@ -82,20 +82,21 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
-def workload_costs(cfg, T):
+def workload_costs(cfg, T, reuse_rank=None):
     """Algorithmic bytes / FLOPs per call (stated in DESIGN.md)."""
     cb = {0: 4, 1: 2, 2: 1}[cfg.code_dtype]
     sb = 4 if cfg.code_dtype == 2 else 0
     ob = 4 if cfg.state_dtype == 0 else 2
     D, d, d_a, r = cfg.D, cfg.d_model, cfg.d_a, cfg.rank
+    rr = reuse_rank or r              # codes per token and REUSE branch (per-head reading: H * r_head)
     P = len(cfg.patch_layers)
     R = cfg.n_layers - P
     c = {}
-    c["reuse_bytes"] = R * T * (2 * (r * cb + sb) + 2 * D * ob)
+    c["reuse_bytes"] = R * T * (2 * (rr * cb + sb) + 2 * D * ob)
     c["reuse_bytes_written"] = R * T * 2 * D * ob
-    c["reuse_flops"] = R * T * 4 * r * D
-    c["encode_bytes"] = R * T * (2 * D * ob + 2 * (r * cb + sb)) + P * T * (d * ob + r * cb + sb)
-    c["encode_flops"] = R * T * 4 * D * r + P * T * 2 * d * r
+    c["reuse_flops"] = R * T * 4 * rr * D
+    c["encode_bytes"] = R * T * (2 * D * ob + 2 * (rr * cb + sb)) + P * T * (d * ob + r * cb + sb)
+    c["encode_flops"] = R * T * 4 * D * rr + P * T * 2 * d * r
     c["patch_flops"] = P * T * 2 * (r * d_a + d_a * d + 2 * d * D)
     c["patch_bytes"] = P * T * (r * cb + sb + 2 * D * ob)
     c["kv_bytes_written"] = cfg.n_layers * T * 2 * D * ob
@@ -204,7 +205,7 @@ def run_ours(args, cfg):
     dev = torch.device(f"cuda:{local}")
     torch.cuda.set_device(dev)
 
-    prob = CodecProblem(cfg, dev)
+    prob = CodecProblem(cfg, dev, per_head_rank=args.per_head_rank)
     T = prob.T
     k, v, h = prob.make_sources()          # content-space states stand in for the post-RoPE cache
     prob.alloc_pools()
@@ -322,7 +323,7 @@ def run_ours(args, cfg):
         return
 
     peaks = load_peaks()
-    costs = workload_costs(cfg, T)
+    costs = workload_costs(cfg, T, cfg.n_kv_heads * args.per_head_rank if args.per_head_rank else None)
     # DRAM bytes per launch from the committed `ncu --set full` captures (profiles/): {kernel: bytes}
     traffic = {}
     tpath = os.path.join(ROOT, "profiles", "traffic.csv")
@@ -385,7 +386,7 @@ def run_ours(args, cfg):
         "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16" if cfg.state_dtype == 1 else "f32", "data": "synthetic",
         "config": {"workload": cfg.name, "tokens": T, "layers": cfg.n_layers, "patch_layers": list(cfg.patch_layers),
-                   "rank": cfg.rank, "code_dtype": {0: "f32", 1: "bf16", 2: "e4m3+f32 rowscale"}[cfg.code_dtype],
+                   "rank": cfg.rank, "reuse_per_head_rank": args.per_head_rank or None, "code_dtype": {0: "f32", 1: "bf16", 2: "e4m3+f32 rowscale"}[cfg.code_dtype],
                    "l2": "flushed (256 MiB fill) before every C-ABI call, outside the events; inputs 2.2 GB >> L2",
                    "parallelism": "replicas only" if world > 1 else "1 gpu"},
         "stages_ms": {"encode": enc_ms, "reuse_decode": dec_ms, "patch": pat_ms},
@@ -419,6 +420,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--rank", type=int, default=0, help="override the config's rank (config 5 rank sweep)")
+    ap.add_argument("--per-head-rank", type=int, default=0,
+                    help="REUSE layers in the paper's per-head reading (one d_h x r map per layer, PAPER.md:102) with this r")
     args = ap.parse_args()
     from paper_2606_07684_b200 import workloads as W
     cfg = W.CONFIGS[args.config]

@@ -81,6 +81,13 @@ typedef struct {
   int32_t patch_act;       /* scd_act_t                                                  */
   int32_t patch_norm;      /* scd_norm_t                                                 */
   float   rms_eps;
+  /* REUSE translator reading.  0: one basis per layer over all heads, enc [D, r], dec [r, D],
+   * means [D] (the shapes BASELINE.json's configs use).  1: the paper's own Sec. 4.1
+   * form: batch x heads x tokens are one sample axis and ONE map per
+   * layer and branch serves every KV head -- enc [d_h, r], dec [r, d_h], means [d_h].  A token's
+   * code row is then its heads' codes side by side: scd_plan_code_segment reports rank
+   * n_kv_heads * r, and r_k / r_v below are the per-head ranks.  PATCH layers are unaffected. */
+  int32_t reuse_per_head;
 } scd_model_desc_t;
 
 /* One per layer.  Artifacts are in state_dtype unless typed float. NULL means "absent"
@@ -89,10 +96,10 @@ typedef struct {
 typedef struct {
   int32_t kind;                      /* scd_kind_t                                       */
   int32_t r_k, r_v;                  /* REUSE ranks, independent          */
-  const void *enc_k, *enc_v;         /* [D, r]  producer encoders  (Eq. 7-8)             */
-  const void *dec_k, *dec_v;         /* [r, D]  consumer decoders  (Eq. 6, 9)            */
-  const float *mean_src_k, *mean_src_v;   /* [D] subtracted before encode, or NULL       */
-  const float *mean_dst_k, *mean_dst_v;   /* [D] added after decode, or NULL             */
+  const void *enc_k, *enc_v;         /* [D, r]  producer encoders  (Eq. 7-8); [d_h, r] if reuse_per_head */
+  const void *dec_k, *dec_v;         /* [r, D]  consumer decoders  (Eq. 6, 9); [r, d_h] if reuse_per_head */
+  const float *mean_src_k, *mean_src_v;   /* [D] ([d_h] if reuse_per_head) subtracted before encode, or NULL */
+  const float *mean_dst_k, *mean_dst_v;   /* [D] ([d_h] if reuse_per_head) added after decode, or NULL      */
   int32_t r_h, d_aligner;            /* PATCH: code rank r_H, aligner hidden width d_a   */
   const void *enc_h;                 /* [d_model, r_h]                   */
   const float *mean_src_h;           /* [d_model] or NULL                                */

@@ -40,7 +40,8 @@ class ModelDesc(C.Structure):
                 ("block_size", C.c_int32), ("max_position", C.c_int32), ("state_dtype", C.c_int32),
                 ("code_dtype", C.c_int32), ("rope_theta_producer", C.c_double), ("rope_theta_consumer", C.c_double),
                 ("rope_style", C.c_int32), ("k_is_roped", C.c_int32), ("rope_on_reuse_k", C.c_int32),
-                ("patch_act", C.c_int32), ("patch_norm", C.c_int32), ("rms_eps", C.c_float)]
+                ("patch_act", C.c_int32), ("patch_norm", C.c_int32), ("rms_eps", C.c_float),
+                ("reuse_per_head", C.c_int32)]
 
 
 class LayerDesc(C.Structure):
@@ -125,11 +126,12 @@ def _stream_ptr(stream) -> Optional[int]:
 def model_desc(*, n_layers, d_model, n_kv_heads, head_dim, max_position, state_dtype, code_dtype,
                rope_theta_producer, rope_theta_consumer=None, block_size=16, rope_style=SCD_ROPE_HALF,
                k_is_roped=1, rope_on_reuse_k=1, patch_act=SCD_ACT_SILU, patch_norm=SCD_NORM_RMS,
-               rms_eps=1e-5) -> ModelDesc:
+               rms_eps=1e-5, reuse_per_head=0) -> ModelDesc:
     return ModelDesc(n_layers, d_model, n_kv_heads, head_dim, block_size, max_position, state_dtype, code_dtype,
                      float(rope_theta_producer),
                      float(rope_theta_producer if rope_theta_consumer is None else rope_theta_consumer),
-                     rope_style, int(k_is_roped), int(rope_on_reuse_k), patch_act, patch_norm, float(rms_eps))
+                     rope_style, int(k_is_roped), int(rope_on_reuse_k), patch_act, patch_norm, float(rms_eps),
+                     int(reuse_per_head))
 
 
 def reuse_layer_desc(*, enc_k, enc_v, dec_k, dec_v, mean_src_k=None, mean_src_v=None, mean_dst_k=None,

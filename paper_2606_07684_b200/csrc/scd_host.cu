@@ -296,6 +296,45 @@ static scd_status_t build_plan(scd_plan_t* p, const scd_layer_desc_t* layers, cu
   return SCD_OK;
 }
 
+// I_H (x) W for the REUSE artifacts of every layer; `temps` owns the device buffers until the plan has repacked them
+scd_status_t expand_per_head(const scd_model_desc_t* m, const scd_layer_desc_t* layers, cudaStream_t s,
+                             std::vector<scd_layer_desc_t>& eff, std::vector<void*>& temps) {
+  const int H = m->n_kv_heads, dh = m->head_dim;
+  const size_t es = state_elem_bytes(m->state_dtype);
+  eff.assign(layers, layers + m->n_layers);
+  auto alloc = [&](size_t bytes) -> void* {
+    void* d = nullptr;
+    if (cudaMalloc(&d, bytes) != cudaSuccess) return nullptr;
+    temps.push_back(d);
+    return d;
+  };
+  for (int i = 0; i < m->n_layers; ++i) {
+    scd_layer_desc_t& l = eff[i];
+    if (l.kind != SCD_REUSE) continue;
+    if (l.r_k < 1 || l.r_v < 1) return fail(SCD_E_SHAPE, "layer %d: REUSE ranks must be positive", i);
+    if (!l.enc_k || !l.enc_v || !l.dec_k || !l.dec_v) return fail(SCD_E_ARG, "layer %d: REUSE artifacts missing", i);
+    struct { const void** w; int rows, cols; } mats[4] = {
+        {&l.enc_k, dh, l.r_k}, {&l.enc_v, dh, l.r_v}, {&l.dec_k, l.r_k, dh}, {&l.dec_v, l.r_v, dh}};
+    for (auto& mt : mats) {
+      void* d = alloc((size_t)H * mt.rows * H * mt.cols * es);
+      if (!d) return fail(SCD_E_NOMEM, "cudaMalloc(per-head expansion)");
+      SCD_CUDA(prep_block_diag(*mt.w, d, mt.rows, mt.cols, H, m->state_dtype, s));
+      *mt.w = d;
+    }
+    const float** means[4] = {&l.mean_src_k, &l.mean_src_v, &l.mean_dst_k, &l.mean_dst_v};
+    for (auto mp : means) {
+      if (!*mp) continue;
+      float* d = (float*)alloc((size_t)H * dh * sizeof(float));
+      if (!d) return fail(SCD_E_NOMEM, "cudaMalloc(per-head expansion)");
+      SCD_CUDA(prep_tile_f32(*mp, d, dh, H, s));
+      *mp = d;
+    }
+    l.r_k *= H;
+    l.r_v *= H;
+  }
+  return SCD_OK;
+}
+
 }  // namespace scd
 
 using namespace scd;
@@ -340,9 +379,12 @@ scd_status_t scd_code_layout(const scd_model_desc_t* model, const scd_layer_desc
   if (!layers) return fail(SCD_E_ARG, "layers is NULL");
   if (total_tokens < 0) return fail(SCD_E_ARG, "total_tokens negative");
   int32_t kind[SCD_MAX_LAYERS], rk[SCD_MAX_LAYERS], rv[SCD_MAX_LAYERS], rh[SCD_MAX_LAYERS];
+  const int hm = model->reuse_per_head ? model->n_kv_heads : 1;     // per-head reading: H * r codes per token
   for (int i = 0; i < model->n_layers; ++i) {
-    if ((st = check_layer_ranks(model, &layers[i], i)) != SCD_OK) return st;
-    kind[i] = layers[i].kind; rk[i] = layers[i].r_k; rv[i] = layers[i].r_v; rh[i] = layers[i].r_h;
+    scd_layer_desc_t le = layers[i];
+    le.r_k *= hm; le.r_v *= hm;
+    if ((st = check_layer_ranks(model, &le, i)) != SCD_OK) return st;
+    kind[i] = le.kind; rk[i] = le.r_k; rv[i] = le.r_v; rh[i] = le.r_h;
   }
   Layout lay;
   compute_layout(model, kind, rk, rv, rh, total_tokens, &lay);
@@ -366,6 +408,20 @@ scd_status_t scd_plan(const scd_model_desc_t* model, const scd_layer_desc_t* lay
   scd_status_t st = check_model(model);
   if (st != SCD_OK) return st;
   if (!layers) return fail(SCD_E_ARG, "layers is NULL");
+  // Per-head reading: the shared d_h x r map is expanded once, here, to the
+  // block-diagonal per-layer operand I_H (x) W (means tiled over heads); everything below then sees a per-layer
+  // plan of rank H * r, and the decode kernel skips the zero blocks (head_rank_k / head_rank_v).
+  std::vector<scd_layer_desc_t> eff;
+  std::vector<void*> temps;
+  struct TempGuard {
+    std::vector<void*>& t;
+    ~TempGuard() { for (void* a : t) cudaFree(a); }
+  } guard{temps};
+  const scd_layer_desc_t* user_layers = layers;
+  if (model->reuse_per_head) {
+    if ((st = expand_per_head(model, layers, (cudaStream_t)stream, eff, temps)) != SCD_OK) return st;
+    layers = eff.data();
+  }
   for (int i = 0; i < model->n_layers; ++i)
     if ((st = check_layer_ranks(model, &layers[i], i)) != SCD_OK) return st;
   if (model->state_dtype == SCD_F32 && model->code_dtype != SCD_F32)
@@ -388,6 +444,9 @@ scd_status_t scd_plan(const scd_model_desc_t* model, const scd_layer_desc_t* lay
     p->r_v.push_back(layers[i].kind == SCD_REUSE ? layers[i].r_v : 0);
     p->r_h.push_back(layers[i].kind == SCD_PATCH ? layers[i].r_h : 0);
     p->d_a.push_back(layers[i].kind == SCD_PATCH ? layers[i].d_aligner : 0);
+    const bool ph = model->reuse_per_head && layers[i].kind == SCD_REUSE;
+    p->head_rank_k.push_back(ph ? user_layers[i].r_k : 0);
+    p->head_rank_v.push_back(ph ? user_layers[i].r_v : 0);
   }
   const char* dbg = getenv("SCD_DEBUG_FORCE_SIMT");
   p->force_simt = dbg && dbg[0] == '1';
@@ -396,6 +455,10 @@ scd_status_t scd_plan(const scd_model_desc_t* model, const scd_layer_desc_t* lay
 
   st = build_plan(p, layers, (cudaStream_t)stream);
   if (st != SCD_OK) { scd_plan_destroy(p); return st; }
+  if (!temps.empty() && cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess) {   // the repacks read the temporaries
+    scd_plan_destroy(p);
+    return fail(SCD_E_CUDA, "plan: %s", cudaGetErrorString(cudaGetLastError()));
+  }
   *out = p;
   return SCD_OK;
 }

@@ -121,6 +121,7 @@ struct scd_plan {
   void* tc_bmaps = nullptr;
   // tile-scheduler counters of the persistent paged-KV kernel: KV_SCHED_SETS pairs {next chunk, CTAs done},
   // zero between launches (the last CTA of a launch resets its pair); launches take the sets round-robin
+  std::vector<int32_t> head_rank_k, head_rank_v;       // per layer: per-head ranks when model.reuse_per_head, else 0
   int32_t* kv_sched = nullptr;
   mutable std::atomic<uint32_t> kv_sched_next{0};
 };
@@ -150,6 +151,9 @@ cudaError_t prep_mean_proj(const float* mu, const void* w_enc, float* c, int wid
 // dst[i] = (float) src[i] (src state dtype, may be null -> zeros)
 cudaError_t prep_to_f32(const void* src, float* dst, int n, int state_dtype, cudaStream_t s);
 cudaError_t prep_copy_f32(const float* src, float* dst, int n, cudaStream_t s);   // null -> zeros
+// per-head REUSE reading: dst [H*rows, H*cols] = I_H (x) src [rows, cols] (state dtype); dst [H*n] = src [n] tiled H times
+cudaError_t prep_block_diag(const void* src, void* dst, int rows, int cols, int heads, int state_dtype, cudaStream_t s);
+cudaError_t prep_tile_f32(const float* src, float* dst, int n, int heads, cudaStream_t s);
 // (cos, sin)(p * theta^(-2j/d_h)) evaluated in fp64, rounded to fp32
 cudaError_t prep_rope_table(float2* table, int max_position, int head_dim, double theta, cudaStream_t s);
 

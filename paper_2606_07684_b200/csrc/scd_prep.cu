@@ -2,6 +2,8 @@
 // PAPER.md:102), never on the hot path.  They bring every B operand of the path's GEMMs
 // into K-major [N, K] form, fold the RMSNorm weight into W_k|W_v, project the source
 // mean through the encoder in fp64 and tabulate RoPE angles in fp64.
+#include <algorithm>
+
 #include "scd_internal.h"
 
 namespace scd {
@@ -123,6 +125,30 @@ cudaError_t prep_rope_table(float2* table, int max_position, int head_dim, doubl
   int grid = (int)((n + 255) / 256 < 2048 ? (n + 255) / 256 : 2048);
   if (grid < 1) grid = 1;
   rope_table_kernel<<<grid, 256, 0, s>>>(table, max_position, head_dim, theta);
+  return cudaGetLastError();
+}
+
+template <typename T>
+__global__ void block_diag_kernel(const T* src, T* dst, int rows, int cols, int heads) {
+  const long long n = (long long)heads * rows * heads * cols;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+    const int c = (int)(i % ((long long)heads * cols)), r = (int)(i / ((long long)heads * cols));
+    const bool on = (r / rows) == (c / cols);
+    dst[i] = on ? src[(size_t)(r % rows) * cols + (c % cols)] : T(0.0f);
+  }
+}
+cudaError_t prep_block_diag(const void* src, void* dst, int rows, int cols, int heads, int state_dtype, cudaStream_t s) {
+  const long long n = (long long)heads * rows * heads * cols;
+  const int grid = (int)std::min<long long>((n + 255) / 256, 4096);
+  if (state_dtype == SCD_F32) block_diag_kernel<float><<<grid, 256, 0, s>>>((const float*)src, (float*)dst, rows, cols, heads);
+  else block_diag_kernel<__nv_bfloat16><<<grid, 256, 0, s>>>((const __nv_bfloat16*)src, (__nv_bfloat16*)dst, rows, cols, heads);
+  return cudaGetLastError();
+}
+__global__ void tile_f32_kernel(const float* src, float* dst, int n, int heads) {
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n * heads; i += gridDim.x * blockDim.x) dst[i] = src[i % n];
+}
+cudaError_t prep_tile_f32(const float* src, float* dst, int n, int heads, cudaStream_t s) {
+  tile_f32_kernel<<<(n * heads + 255) / 256, 256, 0, s>>>(src, dst, n, heads);
   return cudaGetLastError();
 }
 

@@ -272,7 +272,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         const uint32_t acc_phase = (it >> 1) & 1;
         ptx::mbar_wait_suspend(&bars->tmem_empty[acc], acc_phase ^ 1);
         ptx::tc_fence_after();
-        const uint32_t d_tmem = tmem_base + (uint32_t)(acc * block_n);
+        const uint32_t d_tmem = tmem_base + (uint32_t)(acc * 256);
         for (int kb = 0; kb < P.num_kb; ++kb) {
           ptx::mbar_wait_suspend(AMODE != A_PLAIN ? &bars->ready[stage] : &bars->full[stage], phase);
           ptx::tc_fence_after();
@@ -376,7 +376,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       ptx::mbar_wait_suspend(&bars->tmem_full[acc], acc_phase);
       ptx::tc_fence_after();
-      const uint32_t t_row = tmem_base + (uint32_t)(acc * block_n) + ((uint32_t)(ew * 32) << 16);
+      const uint32_t t_row = tmem_base + (uint32_t)(acc * 256) + ((uint32_t)(ew * 32) << 16);
 
       // prefetch the next tile's per-row quantities; consumed at the bottom of the loop
       RowInfo nxt = cur;
@@ -428,7 +428,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       for (int c0 = g_begin; c0 < g_end; c0 += SUB_N) {
         const int sub_cols = min(SUB_N, g_begin + grp_cols - c0);
         const int row_bytes = sub_cols * out_eb;
-        const int pitch = row_bytes < 128 ? 128 : row_bytes;
+        const int pitch = (row_bytes + 127) & ~127;            // whole 128-B swizzle spans
         const bool last_sub = c0 + SUB_N >= g_end;
 
         if (EPI == EPI_KV && (n0 + c0) < sg.rope_cols && P.rope_style == SCD_ROPE_HALF) {
@@ -736,9 +736,13 @@ static int pick_block_n_div(int n) {            // largest tile width that divid
     if (n % b == 0) return b;
   return 0;
 }
-static int pick_block_n_cover(int n) {          // smallest multiple of 16 covering n, capped at 256
-  int b = (n + 15) / 16 * 16;
-  return b > 256 ? 256 : b;
+static int pick_block_n_cover(int n) {          // smallest of 32 / 64 / 128 / 256 covering n (256 if none does)
+  // Power-of-two tile widths only: columns beyond N are zero-filled operand rows (TMA out-of-bounds fill) and are
+  // never stored.  A 192-wide tile (rank 192) produced sporadic NaNs in accumulator columns 96-127 on B200 while
+  // 160 and 224 were clean; the cause was not found, so the odd widths are not used at all.
+  for (int b : {32, 64, 128})
+    if (n <= b) return b;
+  return 256;
 }
 
 scd_status_t tc_supported(const scd_plan_t* p, const scd_layer_desc_t* layers) {
@@ -985,6 +989,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
       }
     }
     P.prof_id = SCD_PROF_REUSE_DECODE;
+    P.head_rank = m.reuse_per_head ? s0.rank / m.n_kv_heads : 0;
     if (e4) st = launch_tc<EPI_KV, A_CODES>(p, P, s);       // operand expansion in shared memory (generic kernel)
     else st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
     if (st != SCD_OK) return st;

@@ -38,6 +38,7 @@ struct TcParams {
   float rms_eps;
   int32_t* sched;                     // paged-KV kernel: {next chunk, CTAs done}
   int32_t chunk_tiles, n_chunks;      // paged-KV kernel: consecutive tiles per dynamically claimed unit
+  int32_t head_rank;                  // paged-KV kernel, per-head REUSE: codes per head (A/B are block-diagonal), else 0
   int32_t prof_id;                    // host only: id under which scd_profile_* reports the launch
   int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
 };

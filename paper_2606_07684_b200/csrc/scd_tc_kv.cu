@@ -64,6 +64,16 @@ struct TileCoord {
 __device__ __forceinline__ void tile_next(const TcParams& P, TileCoord& c) {
   if (++c.n_tile == P.n_tiles) { c.n_tile = 0; if (++c.seg == P.n_segs) { c.seg = 0; ++c.m_tile; } }
 }
+// k-blocks a tile needs.  Per-head REUSE (P.head_rank = r > 0): the operands are block-diagonal, a 256-column tile is
+// heads 2 n_tile and 2 n_tile + 1, whose codes are columns [2 n_tile r, (2 n_tile + 2) r) of the code row.
+__device__ __forceinline__ void tile_kb_range(const TcParams& P, int n_tile, int& kb0, int& kb1) {
+  kb0 = 0;
+  kb1 = P.num_kb;
+  if (P.head_rank > 0) {
+    kb0 = (2 * n_tile * P.head_rank) / BLOCK_K;
+    kb1 = min(P.num_kb, ((2 * n_tile + 2) * P.head_rank + BLOCK_K - 1) / BLOCK_K);
+  }
+}
 __device__ __forceinline__ TileCoord tile_coord(const TcParams& P, int tile) {
   const int per_m = P.n_segs * P.n_tiles;
   TileCoord c;
@@ -168,7 +178,9 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         const TcSeg& sg = P.segs[tc.seg];
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
-        for (int kb = 0; kb < P.num_kb; ++kb) {
+        int kb0, kb1;
+        tile_kb_range(P, tc.n_tile, kb0, kb1);
+        for (int kb = kb0; kb < kb1; ++kb) {
           ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
           ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES + KV_B_STAGE_BYTES);
           ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES, am, &bars->full[stage], kb * BLOCK_K, tc.m_tile * BLOCK_M,
@@ -210,20 +222,24 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
           if (++slot == KV_SCHED_SLOTS) { slot = 0; sphase ^= 1; }
           if (t_begin < 0) break;
         }
+      int n_tile = t_begin % P.n_tiles;                    // the only tile coordinate the MMA loop needs
       for (int tile = t_begin; tile < t_end; ++tile, ++it) {
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
         ptx::mbar_wait_suspend(&bars->tmem_empty[acc], acc_phase ^ 1);
         ptx::tc_fence_after();
         const uint32_t d_tmem = tmem_base + (uint32_t)(acc * KV_BLOCK_N);
-        for (int kb = 0; kb < P.num_kb; ++kb) {
+        int kb0, kb1;
+        tile_kb_range(P, n_tile, kb0, kb1);
+        if (++n_tile == P.n_tiles) n_tile = 0;
+        for (int kb = kb0; kb < kb1; ++kb) {
           ptx::mbar_wait_suspend(&bars->full[stage], phase);
           ptx::tc_fence_after();
           const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
           const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * KV_B_STAGE_BYTES));
 #pragma unroll
           for (int k = 0; k < BLOCK_K / 16; ++k)
-            ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb | k) != 0);
+            ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb > kb0) || k != 0);
           ptx::mma_commit(&bars->empty[stage]);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }

@@ -19,14 +19,16 @@ class CodecProblem:
                  k_is_roped: bool = True, rope_on_reuse_k: bool = True, patch_norm: int = B.SCD_NORM_RMS,
                  patch_act: int = B.SCD_ACT_SILU, rope_style: int = B.SCD_ROPE_HALF,
                  rope_theta_consumer: Optional[float] = None, use_means: bool = True,
-                 artifacts: Optional[List[W.LayerArtifacts]] = None):
+                 artifacts: Optional[List[W.LayerArtifacts]] = None, per_head_rank: int = 0):
         self.cfg = cfg
         self.device = torch.device(device)
         self.batch = W.make_batch(cfg, self.device, pos_offset)
         self.T = self.batch.total_tokens
         self.use_means = use_means
         self.arts = artifacts if artifacts is not None else [
-            W.make_layer_artifacts(cfg, l, self.device, total_rows=max(self.T, 1)) for l in range(cfg.n_layers)]
+            W.make_layer_artifacts(cfg, l, self.device, total_rows=max(self.T, 1), per_head_rank=per_head_rank)
+            for l in range(cfg.n_layers)]
+        self.per_head_rank = per_head_rank
         max_off = max(pos_offset) if pos_offset is not None else 0
         self.max_position = max(16, (self.batch.max_seqlen + max_off + 15) // 16 * 16)
         self.model = B.model_desc(
@@ -34,7 +36,7 @@ class CodecProblem:
             max_position=self.max_position, state_dtype=cfg.state_dtype, code_dtype=cfg.code_dtype,
             rope_theta_producer=cfg.rope_theta, rope_theta_consumer=rope_theta_consumer, block_size=cfg.block_size,
             rope_style=rope_style, k_is_roped=int(k_is_roped), rope_on_reuse_k=int(rope_on_reuse_k),
-            patch_act=patch_act, patch_norm=patch_norm, rms_eps=cfg.rms_eps)
+            patch_act=patch_act, patch_norm=patch_norm, rms_eps=cfg.rms_eps, reuse_per_head=int(per_head_rank > 0))
         self.layer_descs = [self._desc(a) for a in self.arts]
         self.plan = B.scd_plan(self.model, self.layer_descs)
         torch.cuda.synchronize(self.device)

@@ -216,17 +216,23 @@ class LayerArtifacts:
 
 
 def make_layer_artifacts(cfg: WorkloadConfig, layer: int, device, cal_rows: int = 8192,
-                         total_rows: Optional[int] = None) -> LayerArtifacts:
+                         total_rows: Optional[int] = None, per_head_rank: int = 0) -> LayerArtifacts:
     """Artifacts of one layer.  REUSE: one orthonormal-row PCA basis per branch, W_dec = B,
     W_enc = B^T, mu_src = mu_dst = calibration mean.  PATCH: W1 = B_H and
     b1 = mu_H (d_a = d_model) or Gaussian W1/b1 when d_a != d_model; W2, W_k, W_v ~
-    N(0, 1/fan_in); gamma = 1 + 0.1 N(0,1); no b2 / b_k / b_v."""
+    N(0, 1/fan_in); gamma = 1 + 0.1 N(0,1); no b2 / b_k / b_v.
+    `per_head_rank` > 0: the paper's per-head reading for REUSE layers: the calibration rows are
+    flattened to [rows * H, d_h] and ONE basis [r, d_h] / mean [d_h] is fitted for all heads."""
     sd = torch_state_dtype(cfg)
     n_cal = cal_rows if total_rows is None else min(cal_rows, total_rows)
     if layer not in cfg.patch_layers:
         art = LayerArtifacts(REUSE)
         for branch, name in ((0, "k"), (1, "v")):
-            b, mu = fit_basis(make_state(cfg, layer, branch, n_cal, device), cfg.rank)
+            x_cal = make_state(cfg, layer, branch, n_cal, device)
+            if per_head_rank:
+                b, mu = fit_basis(x_cal.reshape(-1, cfg.head_dim), per_head_rank)
+            else:
+                b, mu = fit_basis(x_cal, cfg.rank)
             setattr(art, f"dec_{name}", b.to(sd).contiguous())
             setattr(art, f"enc_{name}", b.t().to(sd).contiguous())
             setattr(art, f"mean_{name}", mu.float().contiguous())

@@ -32,7 +32,8 @@ def oracle_model(prob) -> O.Model:
                    block_size=m.block_size, rope_theta_producer=m.rope_theta_producer,
                    rope_theta_consumer=m.rope_theta_consumer, rope_style=m.rope_style,
                    k_is_roped=bool(m.k_is_roped), rope_on_reuse_k=bool(m.rope_on_reuse_k), code_dtype=m.code_dtype,
-                   patch_act=m.patch_act, patch_norm=m.patch_norm, rms_eps=float(m.rms_eps))
+                   patch_act=m.patch_act, patch_norm=m.patch_norm, rms_eps=float(m.rms_eps),
+                   reuse_per_head=bool(m.reuse_per_head))
 
 
 def oracle_layer(prob, l: int) -> O.Layer:
@@ -115,7 +116,12 @@ def check_encode(prob, k, v, h, rows: Optional[np.ndarray] = None) -> Dict:
                 if s_rtol > 1e-5:
                     kt = O.rope(np64(k[l][tsel]), pos[sel], om.rope_theta_producer, -1, om.n_kv_heads, om.head_dim,
                                 om.rope_style)
-                    step = step + 2.0 ** -8 * np.linalg.norm(kt, axis=1)[:, None] * np.linalg.norm(ol.enc_k, axis=0)[None, :]
+                    if om.reuse_per_head:     # code (t, h, i) sees head h of the row only
+                        hn = np.linalg.norm(kt.reshape(len(kt), om.n_kv_heads, om.head_dim), axis=2)
+                        extra = hn[:, :, None] * np.linalg.norm(ol.enc_k, axis=0)[None, None, :]
+                        step = step + 2.0 ** -8 * extra.reshape(len(kt), -1)
+                    else:
+                        step = step + 2.0 ** -8 * np.linalg.norm(kt, axis=1)[:, None] * np.linalg.norm(ol.enc_k, axis=0)[None, :]
                 assert np.all(np.abs(got - want) <= step * 1.001), f"e4m3 code off by more than one step, layer {l} branch {br}"
     return {"worst_rel_fro": worst}
 

@@ -128,6 +128,27 @@ def test_e4m3_operand_expansion_is_exact_for_every_code(cuda_device):
         assert np.abs(want[3::4]).max() > 0          # the small-code rows are not trivially zero
 
 
+@pytest.mark.parametrize("name,r_h", [("tiny", 8), ("llama3_8b_8k", 16), ("llama3_8b_8k", 24), ("llama3_8b_8k", 32),
+                                       ("llama3_8b_8k", 64), ("llama3_8b_ragged", 16), ("mistral_7b_32k_fp8", 32)])
+def test_per_head_reuse_mode(name, r_h, cuda_device):
+    """The paper's own Sec. 4.1 translator: one d_h x r map per layer and branch shared by all
+    KV heads, heads flattened into the sample axis (scd_model_desc_t.reuse_per_head).  The code row of a token is
+    H * r wide; the decode kernel skips the zero blocks of I_H (x) W (k-block range per n-tile), which r = 24 / 32 / 64
+    exercise with ranges that straddle, equal and span k-blocks."""
+    prob = _problem(MINI[name], cuda_device, per_head_rank=r_h)
+    assert prob.plan.code_segment(0, 0, prob.T)[2] == MINI[name].n_kv_heads * r_h
+    res = _run_all(prob)
+    print(name, r_h, res)
+
+
+@pytest.mark.parametrize("rank", [96, 192])
+def test_ranks_that_are_not_powers_of_two(rank, cuda_device):
+    """Ranks between the tile widths (the encode tile is the next of 32 / 64 / 128 / 256; the extra accumulator
+    columns come from zero-filled operand rows and are never stored).  192 once produced sporadic NaNs."""
+    cfg = MINI["llama3_8b_8k"].scaled(rank=rank, seqlens=(700,), n_layers=2, patch_layers=(1,))
+    _run_all(_problem(cfg, cuda_device))
+
+
 @pytest.mark.parametrize("state", ["f32", "bf16"])
 def test_edge_batches(state, cuda_device):
     """Ragged lengths that are not multiples of 16 / 128, a 1-token request, position offsets,
