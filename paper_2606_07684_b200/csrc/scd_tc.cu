@@ -534,7 +534,9 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         } else {
           __syncwarp();
         }
-        stg_copy_out(stg, pitch, row_bytes, (n_end - c0) * out_eb, row_ptr, (unsigned long long)c0 * out_eb, lane);
+        // valid bytes: the N tail, and never more than this warp staged (a 96-column group rounds its lanes-per-row
+        // up to 16 chunks; the 4 extra chunks are the other group's columns)
+        stg_copy_out(stg, pitch, row_bytes, min(row_bytes, (n_end - c0) * out_eb), row_ptr, (unsigned long long)c0 * out_eb, lane);
         __syncwarp();
       }
       if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = ss_u;
@@ -736,13 +738,9 @@ static int pick_block_n_div(int n) {            // largest tile width that divid
     if (n % b == 0) return b;
   return 0;
 }
-static int pick_block_n_cover(int n) {          // smallest of 32 / 64 / 128 / 256 covering n (256 if none does)
-  // Power-of-two tile widths only: columns beyond N are zero-filled operand rows (TMA out-of-bounds fill) and are
-  // never stored.  A 192-wide tile (rank 192) produced sporadic NaNs in accumulator columns 96-127 on B200 while
-  // 160 and 224 were clean; the cause was not found, so the odd widths are not used at all.
-  for (int b : {32, 64, 128})
-    if (n <= b) return b;
-  return 256;
+static int pick_block_n_cover(int n) {          // smallest multiple of 16 covering n, capped at 256
+  int b = (n + 15) / 16 * 16;
+  return b > 256 ? 256 : b;
 }
 
 scd_status_t tc_supported(const scd_plan_t* p, const scd_layer_desc_t* layers) {

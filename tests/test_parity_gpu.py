@@ -143,8 +143,8 @@ def test_per_head_reuse_mode(name, r_h, cuda_device):
 
 @pytest.mark.parametrize("rank", [96, 192])
 def test_ranks_that_are_not_powers_of_two(rank, cuda_device):
-    """Ranks between the tile widths (the encode tile is the next of 32 / 64 / 128 / 256; the extra accumulator
-    columns come from zero-filled operand rows and are never stored).  192 once produced sporadic NaNs."""
+    """Tile widths that are not powers of two (the encode tile is the rank rounded up to 16).  192 = two 96-column
+    warp groups once had its copy-out overwrite the neighbouring group's first 32 columns (sporadic NaNs)."""
     cfg = MINI["llama3_8b_8k"].scaled(rank=rank, seqlens=(700,), n_layers=2, patch_layers=(1,))
     _run_all(_problem(cfg, cuda_device))
 
