@@ -226,6 +226,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
+  ptx::grid_dep_wait();                 // the previous kernel of the stream has completed and flushed
+  ptx::grid_dep_launch_dependents();    // the next one may start its prologue as SMs free up
 
   // A_DEROPE: 896 threads x 72 registers, re-dealt per role: control warps 24, epilogue warps 128,
   // rotation warps 56 (= 64512)
@@ -821,7 +823,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   }
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
-  tc_gemm_kernel<EPI, AMODE><<<grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, smem, s>>>(P);
+  launch_pdl(tc_gemm_kernel<EPI, AMODE>, grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, smem, s, P);
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));

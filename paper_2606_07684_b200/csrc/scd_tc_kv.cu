@@ -137,6 +137,8 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
   __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
+  ptx::grid_dep_wait();                 // the previous kernel of the stream has completed and flushed
+  ptx::grid_dep_launch_dependents();    // the next one may start its prologue as SMs free up
 
   if (warp < KV_FIRST_EPI_WARP) {
     ptx::setmaxnreg_dec<32>();   // 128 x 32 + 512 x 112 = 640 x 96: the CTA pool is what the launch allocated
@@ -490,9 +492,9 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
     P.dyn_begin = grid * P.static_tiles;
     P.n_chunks = total - P.dyn_begin;
     P.sched = p->kv_sched + 2 * (p->kv_sched_next.fetch_add(1) % KV_SCHED_SETS);
-    tc_kv_kernel<true><<<grid, KV_NTHREADS, smem, s>>>(P);
+    launch_pdl(tc_kv_kernel<true>, grid, KV_NTHREADS, smem, s, P);
   } else {
-    tc_kv_kernel<false><<<grid, KV_NTHREADS, smem, s>>>(P);
+    launch_pdl(tc_kv_kernel<false>, grid, KV_NTHREADS, smem, s, P);
   }
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
