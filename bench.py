@@ -33,7 +33,7 @@ METRIC = "reconstructed KV tokens/s (REUSE+PATCH hybrid cache, encode->reuse_dec
 UNIT = "tokens/s"
 KERNEL_NAMES = {100: "tc_gemm<codes,plain> (encode V/H)", 101: "tc_gemm<codes,derope> (encode K)",
                 110: "tc_kv_kernel / tc_gemm<paged_kv> (reuse decode)", 120: "tc_gemm<aligner_in> (patch GEMM-1)",
-                130: "tc_gemm<aligner_out> (patch GEMM-2)", 140: "tc_kv_kernel<dyn> (patch GEMM-3)"}
+                130: "tc_gemm<aligner_out> (patch GEMM-2)", 140: "tc_kv_kernel<dyn> (patch GEMM-3)"}     # 120-140: one launch per group of PATCH layers
 
 
 # ------------------------------------------------------------------------------ helpers
@@ -353,21 +353,17 @@ def run_ours(args, cfg):
                                          "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": ach / peaks["hbm_gbs"],
                                          "traffic": traffic.get("reuse_decode"), "ms": call_ms,
                                          "share_of_step": call_ms / step_ms, "write_gbs": wr}
-        elif kid == 140:    # PATCH GEMM-3 (+ row scale, RoPE, paged write): tensor-bound
-            ach = costs["gemm3_flops_per_launch"] / (avg_ms * 1e-3) / 1e12
-            rooflines["patch_gemm3"] = {"kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach,
-                                        "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                                        "frac": ach / peaks["bf16_tflops_sustained"],
-                                        "traffic": traffic.get("patch_gemm3"), "ms": avg_ms,
-                                        "share_of_step": avg_ms * len(cfg.patch_layers) / step_ms}
-        elif kid in (120, 130):
-            fl = costs["gemm1_flops_per_launch"] if kid == 120 else costs["gemm2_flops_per_launch"]
-            ach = fl / (avg_ms * 1e-3) / 1e12
-            rooflines["patch_gemm1" if kid == 120 else "patch_gemm2"] = {
-                "kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach, "peak": peaks["bf16_tflops_sustained"],
-                "unit": "TFLOP/s", "frac": ach / peaks["bf16_tflops_sustained"],
-                "traffic": traffic.get("patch_gemm1" if kid == 120 else "patch_gemm2"), "ms": avg_ms,
-                "share_of_step": avg_ms * len(cfg.patch_layers) / step_ms}
+        elif kid in (120, 130, 140):
+            # PATCH GEMM-1 / GEMM-2 / GEMM-3: a launch covers a group of PATCH layers (one segment per layer), so the
+            # algorithmic FLOPs per launch are the per-layer figure x layers per launch; `ms` is the launch average
+            name = {120: "patch_gemm1", 130: "patch_gemm2", 140: "patch_gemm3"}[kid]
+            per_layer = costs[{120: "gemm1_flops_per_launch", 130: "gemm2_flops_per_launch", 140: "gemm3_flops_per_launch"}[kid]]
+            layers_per_launch = len(cfg.patch_layers) / per_pass
+            ach = per_layer * layers_per_launch / (avg_ms * 1e-3) / 1e12
+            rooflines[name] = {"kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach,
+                               "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
+                               "frac": ach / peaks["bf16_tflops_sustained"], "traffic": traffic.get(name), "ms": avg_ms,
+                               "layers_per_launch": layers_per_launch, "share_of_step": avg_ms * per_pass / step_ms}
         elif kid in (100, 101):
             pass
     if enc_ms > 0:

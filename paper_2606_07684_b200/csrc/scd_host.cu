@@ -135,15 +135,32 @@ static void plan_layout(const scd_plan_t* p, int32_t T, Layout* lay) {
   compute_layout(&p->model, p->kind.data(), p->r_k.data(), p->r_v.data(), p->r_h.data(), T, lay);
 }
 
-static size_t patch_workspace(const scd_plan_t* p, int32_t T) {
-  if (p->patches.empty() || T <= 0) return 0;
+// scd_patch workspace: `group` slices of {a [T, d_a], u [T, d], sum-of-squares partials}.  The tensor-core path runs
+// each GEMM stage of up to `group` PATCH layers as one multi-segment launch (fewer launches, fuller last wave); the
+// group is as many layers as fit in 2 GiB of workspace (at least 1, at most 16).
+struct PatchWs {
+  size_t act_stride = 0, u_stride = 0, ss_stride = 0;
+  int group = 1;
+  size_t total() const { return (size_t)group * (act_stride + u_stride + ss_stride); }
+};
+static PatchWs patch_ws(const scd_plan_t* p, int32_t T) {
+  PatchWs w;
+  if (p->patches.empty() || T <= 0) { w.group = 0; return w; }
   const size_t es = state_elem_bytes(p->model.state_dtype);
   int d_a = 0;
   for (auto& pp : p->patches) d_a = pp.d_a > d_a ? pp.d_a : d_a;
   const int d = p->model.d_model;
-  return align_up((size_t)T * d_a * es, 128) + align_up((size_t)T * d * es, 128) +
-         align_up((size_t)(2 * ((d + 127) / 128)) * T * 4, 128);   // sum-of-squares partials
+  w.act_stride = align_up((size_t)T * d_a * es, 128);
+  w.u_stride = align_up((size_t)T * d * es, 128);
+  w.ss_stride = align_up((size_t)(2 * ((d + 127) / 128)) * T * 4, 128);   // sum-of-squares partials
+  const size_t per_layer = w.act_stride + w.u_stride + w.ss_stride;
+  size_t g = p->use_tc ? ((size_t)2 << 30) / per_layer : 1;
+  g = g < 1 ? 1 : g;
+  g = g > 16 ? 16 : g;
+  w.group = (int)(g > p->patches.size() ? p->patches.size() : g);
+  return w;
 }
+static size_t patch_workspace(const scd_plan_t* p, int32_t T) { return patch_ws(p, T).total(); }
 
 // ---------------------------------------------------------------------------------
 // batch validation shared by the hot calls
@@ -626,12 +643,15 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
   int d_a_max = 0;
   for (auto& pp : plan->patches) d_a_max = pp.d_a > d_a_max ? pp.d_a : d_a_max;
   const int d = m.d_model, D = plan->D;
+  const PatchWs pw = patch_ws(plan, T);
   char* ws_act = (char*)workspace;
-  char* ws_u = ws_act + align_up((size_t)T * d_a_max * es, 128);
-  float* ws_ss = (float*)(ws_u + align_up((size_t)T * d * es, 128));
+  char* ws_u = ws_act + (size_t)pw.group * pw.act_stride;
+  float* ws_ss = (float*)(ws_u + (size_t)pw.group * pw.u_stride);
+  (void)es; (void)d_a_max;
 
   if (plan->use_tc)
-    return tc_patch(plan, batch, codes, kv, ws_act, ws_u, ws_ss, lay.off, lay.soff, (cudaStream_t)stream);
+    return tc_patch(plan, batch, codes, kv, ws_act, ws_u, ws_ss, pw.group, pw.act_stride, pw.u_stride, pw.ss_stride, lay.off,
+                    lay.soff, (cudaStream_t)stream);
 
   BatchDev bd = batch_dev(plan, batch, true);
   RopeDev rd = rope_dev(plan, false);

@@ -1003,51 +1003,81 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
 }
 
 // ---------------------------------------------------------------------------------
-// scd_patch on tensor cores: per PATCH layer  GEMM-1 (aligner in) -> GEMM-2 (aligner out,
-// row sum of squares) -> GEMM-3 ([gamma.W_k | gamma.W_v], row scale, RoPE, paged write)
+// scd_patch on tensor cores: GEMM-1 (aligner in) -> GEMM-2 (aligner out, row sum of squares) -> GEMM-3
+// ([gamma.W_k | gamma.W_v], row scale, RoPE, paged write).  PATCH layers are independent of one another
+// (Alg. 1), so each stage runs for a GROUP of layers as one multi-segment launch: three
+// launches per group instead of three per layer, and GEMM-3's 512 tiles per layer (3.46 waves on 148 SMs)
+// become 512 x group tiles.  A group = consecutive PATCH layers of equal (r_h, d_a), at most `group` of them
+// (what the workspace holds).
 // ---------------------------------------------------------------------------------
 scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void* codes, const scd_paged_kv_t* kv,
-                      void* ws_act, void* ws_u, float* ws_ss, const size_t* off, const size_t* soff, cudaStream_t s) {
+                      void* ws_act, void* ws_u, float* ws_ss, int group, size_t act_stride, size_t u_stride, size_t ss_stride,
+                      const size_t* off, const size_t* soff, cudaStream_t s) {
   const scd_model_desc_t& m = p->model;
   const int T = batch->total_tokens, d = m.d_model, D = p->D;
   const bool e4 = m.code_dtype == SCD_E4M3_ROWSCALE;
   const bool rms = m.patch_norm == SCD_NORM_RMS;
   const int nseg = (int)p->segs.size();
   scd_status_t st;
-  for (size_t j = 0; j < p->patches.size(); ++j) {
-    const PatchPlan& pp = p->patches[j];
-    const int key = pp.layer * 3 + SCD_BRANCH_H;
+  if (group < 1) group = 1;
+  if (group > TC_MAX_SEGS) group = TC_MAX_SEGS;
+  size_t j0 = 0;
+  while (j0 < p->patches.size()) {
+    size_t j1 = j0;
+    while (j1 < p->patches.size() && j1 - j0 < (size_t)group && p->patches[j1].r_h == p->patches[j0].r_h &&
+           p->patches[j1].d_a == p->patches[j0].d_a)
+      ++j1;
+    const PatchPlan& p0 = p->patches[j0];
+    const int g = (int)(j1 - j0);
     static thread_local TcParams P;
-    // GEMM-1: [T, r_h] x [r_h, d_a]
+    // GEMM-1: [T, r_h] x [r_h, d_a] per layer
     fill_common(p, batch, true, false, P);
-    P.n_segs = 1; P.N = pp.d_a; P.K = pp.r_h; P.block_n = pick_block_n_cover(pp.d_a);
-    st = e4 ? make_code_map_u8(&P.a_maps[0], (const char*)codes + off[key], pp.r_h, T, 1, align_up((size_t)T * pp.r_h, 128))
-            : make_map(&P.a_maps[0], (const char*)codes + off[key], pp.r_h, T, 1, (uint64_t)pp.r_h * 2,
-                       align_up((size_t)T * pp.r_h * 2, 128), BLOCK_M, 1);
-    if (st != SCD_OK) return st;
-    P.segs[0].col_vec = pp.b1; P.segs[0].out0 = ws_act; P.segs[0].b_map = 2 * nseg + 3 * (int)j;
-    P.segs[0].a_scale = e4 ? (const float*)((const char*)codes + soff[key]) : nullptr;
+    P.n_segs = g; P.N = p0.d_a; P.K = p0.r_h; P.block_n = pick_block_n_cover(p0.d_a);
+    for (int q = 0; q < g; ++q) {
+      const PatchPlan& pp = p->patches[j0 + q];
+      const int key = pp.layer * 3 + SCD_BRANCH_H;
+      st = e4 ? make_code_map_u8(&P.a_maps[q], (const char*)codes + off[key], pp.r_h, T, 1, align_up((size_t)T * pp.r_h, 128))
+              : make_map(&P.a_maps[q], (const char*)codes + off[key], pp.r_h, T, 1, (uint64_t)pp.r_h * 2,
+                         align_up((size_t)T * pp.r_h * 2, 128), BLOCK_M, 1);
+      if (st != SCD_OK) return st;
+      TcSeg& sg = P.segs[q];
+      sg.a_map = q; sg.col_vec = pp.b1; sg.out0 = (char*)ws_act + q * act_stride; sg.b_map = 2 * nseg + 3 * (int)(j0 + q);
+      sg.a_scale = e4 ? (const float*)((const char*)codes + soff[key]) : nullptr;
+    }
     P.prof_id = SCD_PROF_PATCH_GEMM1;
     if ((st = e4 ? launch_tc<EPI_ACT, A_CODES>(p, P, s) : launch_tc<EPI_ACT, A_PLAIN>(p, P, s)) != SCD_OK) return st;
-    // GEMM-2: [T, d_a] x [d_a, d]
+    // GEMM-2: [T, d_a] x [d_a, d] per layer
     fill_common(p, batch, true, false, P);
-    P.n_segs = 1; P.N = d; P.K = pp.d_a; P.block_n = pick_block_n_cover(d);
-    if ((st = make_map(&P.a_maps[0], ws_act, pp.d_a, T, 1, (uint64_t)pp.d_a * 2, (uint64_t)pp.d_a * 2 * T, BLOCK_M, 1)) != SCD_OK) return st;
-    P.segs[0].col_vec = pp.b2; P.segs[0].out0 = ws_u; P.segs[0].aux = rms ? ws_ss : nullptr;
-    P.segs[0].b_map = 2 * nseg + 3 * (int)j + 1;
+    P.n_segs = g; P.N = d; P.K = p0.d_a; P.block_n = pick_block_n_cover(d);
     const int n_partials = 2 * ((d + P.block_n - 1) / P.block_n);   // two column groups per n-tile
+    for (int q = 0; q < g; ++q) {
+      const PatchPlan& pp = p->patches[j0 + q];
+      if ((st = make_map(&P.a_maps[q], (char*)ws_act + q * act_stride, pp.d_a, T, 1, (uint64_t)pp.d_a * 2,
+                         (uint64_t)pp.d_a * 2 * T, BLOCK_M, 1)) != SCD_OK) return st;
+      TcSeg& sg = P.segs[q];
+      sg.a_map = q; sg.col_vec = pp.b2; sg.out0 = (char*)ws_u + q * u_stride;
+      sg.aux = rms ? (float*)((char*)ws_ss + q * ss_stride) : nullptr;
+      sg.b_map = 2 * nseg + 3 * (int)(j0 + q) + 1;
+    }
     P.prof_id = SCD_PROF_PATCH_GEMM2;
     if ((st = launch_tc<EPI_U, A_PLAIN>(p, P, s)) != SCD_OK) return st;
-    // GEMM-3: [T, d] x [d, 2D]
+    // GEMM-3: [T, d] x [d, 2D] per layer
     fill_common(p, batch, true, false, P);
-    P.n_segs = 1; P.N = 2 * D; P.K = d; P.block_n = pick_block_n_div(D);
+    P.n_segs = g; P.N = 2 * D; P.K = d; P.block_n = pick_block_n_div(D);
     P.split = D; P.pool_width = D; P.n_partials = n_partials; P.rms_dim = d; P.rms_eps = m.rms_eps;
-    if ((st = make_map(&P.a_maps[0], ws_u, d, T, 1, (uint64_t)d * 2, (uint64_t)d * 2 * T, BLOCK_M, 1)) != SCD_OK) return st;
-    P.segs[0].col_vec = pp.bkv; P.segs[0].out0 = kv->k_pool[pp.layer]; P.segs[0].out1 = kv->v_pool[pp.layer];
-    P.segs[0].rowscale_in = rms ? ws_ss : nullptr; P.segs[0].rope_cols = D;
-    P.segs[0].b_map = 2 * nseg + 3 * (int)j + 2;
+    for (int q = 0; q < g; ++q) {
+      const PatchPlan& pp = p->patches[j0 + q];
+      if ((st = make_map(&P.a_maps[q], (char*)ws_u + q * u_stride, d, T, 1, (uint64_t)d * 2, (uint64_t)d * 2 * T, BLOCK_M, 1)) != SCD_OK)
+        return st;
+      TcSeg& sg = P.segs[q];
+      sg.a_map = q; sg.col_vec = pp.bkv; sg.out0 = kv->k_pool[pp.layer]; sg.out1 = kv->v_pool[pp.layer];
+      sg.rowscale_in = rms ? (const float*)((const char*)ws_ss + q * ss_stride) : nullptr;
+      sg.rope_cols = D;
+      sg.b_map = 2 * nseg + 3 * (int)(j0 + q) + 2;
+    }
     P.prof_id = SCD_PROF_PATCH_GEMM3;
     if ((st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
+    j0 = j1;
   }
   return SCD_OK;
 }

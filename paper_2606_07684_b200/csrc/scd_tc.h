@@ -18,6 +18,7 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
 scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, const void* codes,
                              const scd_paged_kv_t* kv, const size_t* off, const size_t* soff, cudaStream_t s);
 scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void* codes, const scd_paged_kv_t* kv,
-                      void* ws_act, void* ws_u, float* ws_ss, const size_t* off, const size_t* soff, cudaStream_t s);
+                      void* ws_act, void* ws_u, float* ws_ss, int group, size_t act_stride, size_t u_stride, size_t ss_stride,
+                      const size_t* off, const size_t* soff, cudaStream_t s);
 
 }  // namespace scd

@@ -61,8 +61,19 @@ __device__ __forceinline__ uint32_t qstg_addr(uint32_t stg, int row, int chunk) 
 struct TileCoord {
   int m_tile, seg, n_tile;
 };
+// Tile order.  SEG_SLOWEST = false (REUSE decode): (m-tile, segment, n-tile) -- a CTA's contiguous share stays on a
+// handful of m-tiles, so per-row state is computed once for all layers.  SEG_SLOWEST = true (PATCH GEMM-3 over a group
+// of layers): (segment, m-tile, n-tile) -- one layer's 33 MB weight slab at a time stays L2-resident.
+template <bool SEG_SLOWEST>
 __device__ __forceinline__ void tile_next(const TcParams& P, TileCoord& c) {
-  if (++c.n_tile == P.n_tiles) { c.n_tile = 0; if (++c.seg == P.n_segs) { c.seg = 0; ++c.m_tile; } }
+  if (++c.n_tile == P.n_tiles) {
+    c.n_tile = 0;
+    if (SEG_SLOWEST) {
+      if (++c.m_tile == P.m_tiles) { c.m_tile = 0; ++c.seg; }
+    } else {
+      if (++c.seg == P.n_segs) { c.seg = 0; ++c.m_tile; }
+    }
+  }
 }
 // k-blocks a tile needs.  Per-head REUSE (P.head_rank = r > 0): the operands are block-diagonal, a 256-column tile is
 // heads 2 n_tile and 2 n_tile + 1, whose codes are columns [2 n_tile r, (2 n_tile + 2) r) of the code row.
@@ -74,13 +85,22 @@ __device__ __forceinline__ void tile_kb_range(const TcParams& P, int n_tile, int
     kb1 = min(P.num_kb, ((2 * n_tile + 2) * P.head_rank + BLOCK_K - 1) / BLOCK_K);
   }
 }
+template <bool SEG_SLOWEST>
 __device__ __forceinline__ TileCoord tile_coord(const TcParams& P, int tile) {
-  const int per_m = P.n_segs * P.n_tiles;
   TileCoord c;
-  c.m_tile = tile / per_m;
-  const int rem = tile - c.m_tile * per_m;
-  c.seg = rem / P.n_tiles;
-  c.n_tile = rem - c.seg * P.n_tiles;
+  if (SEG_SLOWEST) {
+    const int per_seg = P.m_tiles * P.n_tiles;
+    c.seg = tile / per_seg;
+    const int rem = tile - c.seg * per_seg;
+    c.m_tile = rem / P.n_tiles;
+    c.n_tile = rem - c.m_tile * P.n_tiles;
+  } else {
+    const int per_m = P.n_segs * P.n_tiles;
+    c.m_tile = tile / per_m;
+    const int rem = tile - c.m_tile * per_m;
+    c.seg = rem / P.n_tiles;
+    c.n_tile = rem - c.seg * P.n_tiles;
+  }
   return c;
 }
 
@@ -175,8 +195,8 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         if (++slot == KV_SCHED_SLOTS) { slot = 0; sphase ^= 1; }
         if (t_begin < 0) break;
         }
-      TileCoord tc = tile_coord(P, t_begin);
-      for (int tile = t_begin; tile < t_end; ++tile, tile_next(P, tc)) {
+      TileCoord tc = tile_coord<DYN>(P, t_begin);
+      for (int tile = t_begin; tile < t_end; ++tile, tile_next<DYN>(P, tc)) {
         const TcSeg& sg = P.segs[tc.seg];
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
@@ -259,8 +279,8 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
     const uint32_t wvec = ptx::smem_u32(smem_vec) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 256;
     const uint32_t bar_id = 1 + q;
 
-    // per-row state, recomputed when the m-tile changes
-    int cur_m = -1;
+    // per-row state, recomputed when the m-tile changes (DYN: or the segment -- the RMS scale belongs to a layer)
+    int cur_m = -1, cur_seg = -1;
     unsigned long long slot_off = 0;                          // byte offset of the row's slot inside a pool
     bool valid = false;
     float rs_row = 1.0f;
@@ -308,19 +328,20 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         if (t_begin < 0) break;
       }
     Pre cur;
-    TileCoord tc = tile_coord(P, t_begin);
+    TileCoord tc = tile_coord<DYN>(P, t_begin);
     if (t_begin < t_end) cur = fetch(tc);
     for (int tile = t_begin; tile < t_end; ++tile, ++it) {
       TileCoord tn = tc;
-      tile_next(P, tn);
+      tile_next<DYN>(P, tn);
       const TcSeg& sg = P.segs[tc.seg];
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
       const int n0 = tc.n_tile * KV_BLOCK_N;
       const bool is_k = n0 < sg.rope_cols;
 
-      if (tc.m_tile != cur_m) {
+      if (tc.m_tile != cur_m || (DYN && tc.seg != cur_seg)) {
         cur_m = tc.m_tile;
+        cur_seg = tc.seg;
         const int row = cur_m * BLOCK_M + q * 32 + lane;
         valid = row < P.M;
         int pos = 0;
@@ -328,7 +349,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         rs_row = 1.0f;
         if (valid) {
           row_to_pos_slot(P.batch, row, pos, slot);
-          if (sg.rowscale_in) {                                 // NORM_RMS (PATCH GEMM-3; single segment)
+          if (sg.rowscale_in) {                                 // NORM_RMS (PATCH GEMM-3; several segments only with DYN)
             float ss = 0.0f;
             for (int p = 0; p < P.n_partials; ++p) ss += __ldg(sg.rowscale_in + (size_t)p * P.M + row);
             rs_row = rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
@@ -461,7 +482,6 @@ bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P, long long pool_slots
   if (P.block_n != KV_BLOCK_N || (P.N % KV_BLOCK_N) || (P.split % KV_BLOCK_N) || P.a_kb_per_head != 0) return false;
   for (int i = 0; i < P.n_segs; ++i) {
     if (P.segs[i].rope_cols % KV_BLOCK_N) return false;
-    if (P.segs[i].rowscale_in && P.n_segs != 1) return false;
   }
   return true;
 }
@@ -484,7 +504,9 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   const int grid = std::min(total, p->sm_count);
   // long tiles (K = d_model: PATCH GEMM-3): KV_STATIC_PCT % of an even split is owned statically, the rest is
   // claimed tile by tile; short tiles (REUSE decode): static split only
-  const bool dyn = P.num_kb >= 16 && total > grid;
+  bool multi_rowscale = false;                              // several layers' RMS scales: only the DYN variant tracks the segment
+  for (int i = 0; i < P.n_segs; ++i) multi_rowscale |= P.n_segs > 1 && P.segs[i].rowscale_in != nullptr;
+  const bool dyn = (P.num_kb >= 16 && total > grid) || multi_rowscale;
   prof_begin(s);
   if (dyn) {
     P.chunk_tiles = 1;
