@@ -244,7 +244,25 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         const TcSeg& sg = P.segs[seg_i];
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
+        // the A operand streams from HBM: its k-block `pf` steps ahead (this tile's, or the next tile's) is pulled
+        // into L2 now, so that the few shared-memory stages see L2 latency instead of HBM latency
+        const int pf = P.a_prefetch < P.num_kb ? P.a_prefetch : P.num_kb;
+        int nm_tile = 0, nn_tile = 0, nseg_i = 0;
+        const bool has_next = tile + (int)gridDim.x < total_tiles;
+        if (pf > 0 && has_next) tile_decode(P, tile + gridDim.x, nm_tile, nn_tile, nseg_i);
         for (int kb = 0; kb < P.num_kb; ++kb) {
+          if (pf > 0) {
+            const bool same = kb + pf < P.num_kb;
+            if (same || has_next) {
+              const int pkb = same ? kb + pf : kb + pf - P.num_kb;
+              const int pm = same ? m_tile : nm_tile;
+              const TcSeg& ps = same ? sg : P.segs[nseg_i];
+              if (P.a_kb_per_head > 0)
+                ptx::tma_prefetch_l2_3d(&P.a_maps[ps.a_map], (pkb % P.a_kb_per_head) * BLOCK_K, pkb / P.a_kb_per_head, pm * BLOCK_M);
+              else
+                ptx::tma_prefetch_l2_3d(&P.a_maps[ps.a_map], pkb * BLOCK_K, pm * BLOCK_M, ps.a_z);
+            }
+          }
           ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
           // A_CODES: the raw e4m3 tile [128 x 64 B] lands in the upper half of the stage and is expanded in place
           ptx::mbar_expect_tx(&bars->full[stage], (AMODE == A_CODES ? A_STAGE_BYTES / 2 : A_STAGE_BYTES) + b_stage_bytes);
@@ -739,6 +757,9 @@ static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, i
   return SCD_OK;
 }
 
+#ifndef TC_A_PREFETCH
+#define TC_A_PREFETCH 4
+#endif
 static int pick_block_n_div(int n) {            // largest tile width that divides n (paged / split epilogues)
   for (int b : {256, 128, 64, 32})
     if (n % b == 0) return b;
@@ -812,6 +833,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   if (total <= 0) return SCD_OK;
   P.stages = tc_pick_stages(P.block_n, P.num_kb, AMODE == A_DEROPE);   // deRoPE pairs k-blocks
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
+  P.a_prefetch = (EPI == EPI_CODES) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
   P.msb = P.m_tiles;
   if (P.n_tiles > 1) {
     const long long a_tile_bytes = (long long)BLOCK_M * P.K * 2;
