@@ -37,17 +37,24 @@ struct __align__(8) TcBarriers {
   uint32_t tmem_base;
 };
 
-static size_t tc_smem_bytes(int block_n, int stages) {
-  return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) +
-         EPI_WARPS * (STG_WARP_BYTES + VEC_WARP_BYTES) + sizeof(TcBarriers);
+// per-warp staging the epilogue needs: 32 rows x the widest sub-tile row, in whole 128-B swizzle spans.  The encode
+// epilogue (narrow code tiles) needs half of STG_WARP_BYTES; the shared memory it leaves buys a pipeline stage.
+static int tc_stg_warp_bytes(int epi, int block_n) {
+  if (epi != EPI_CODES) return STG_WARP_BYTES;
+  const int cols = (block_n % 64) == 0 ? block_n / 2 : block_n;      // the warp pair splits the columns (gran = 32)
+  const int sub = cols < SUB_N ? cols : SUB_N;
+  return 32 * ((sub * 2 + 127) & ~127);
 }
-static int tc_pick_stages(int block_n, int num_kb, bool even) {
-  const size_t budget = 232448 - 1024 - EPI_WARPS * (STG_WARP_BYTES + VEC_WARP_BYTES) - sizeof(TcBarriers);
+static size_t tc_smem_bytes(int block_n, int stages, int stg_warp_bytes) {
+  return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) +
+         EPI_WARPS * (stg_warp_bytes + VEC_WARP_BYTES) + sizeof(TcBarriers);
+}
+static int tc_pick_stages(int block_n, int num_kb, int stg_warp_bytes) {
+  const size_t budget = 232448 - 1024 - EPI_WARPS * (stg_warp_bytes + VEC_WARP_BYTES) - sizeof(TcBarriers);
   int st = (int)(budget / (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2));
   st = st > MAX_STAGES ? MAX_STAGES : st;
   if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty
-  if (even && (st & 1)) --st;                                                  // deRoPE pairs k-blocks: keep it even
-  return st < 2 ? 2 : st;
+  return st < 2 ? 2 : st;          // odd rings are fine for deRoPE: a k-block pair may straddle the wrap
 }
 
 
@@ -200,7 +207,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
   uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
-  uint8_t* smem_vec = smem_stg + EPI_WARPS * STG_WARP_BYTES;
+  uint8_t* smem_vec = smem_stg + EPI_WARPS * P.stg_warp_bytes;
   TcBarriers* bars = (TcBarriers*)(smem_vec + EPI_WARPS * VEC_WARP_BYTES);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -319,7 +326,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     const int ew = (warp - 4) & 3;                    // TMEM lane quadrant (= warp % 4)
     const int grp = (warp - 4) >> 2;                  // group 0 / 1
     const int half = P.head_dim / 2;
-    const uint32_t stg = ptx::smem_u32(smem_stg + (warp - 4) * STG_WARP_BYTES);
+    const uint32_t stg = ptx::smem_u32(smem_stg + (warp - 4) * P.stg_warp_bytes);
     const uint32_t wvec = ptx::smem_u32(smem_vec + (warp - 4) * VEC_WARP_BYTES);
     const int out_eb = (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2;
     // column split only when both halves keep whole heads (RoPE) and whole 32-column TMEM chunks
@@ -831,7 +838,8 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.num_kb = (P.K + BLOCK_K - 1) / BLOCK_K;
   const int total = P.n_segs * P.m_tiles * P.n_tiles;
   if (total <= 0) return SCD_OK;
-  P.stages = tc_pick_stages(P.block_n, P.num_kb, AMODE == A_DEROPE);   // deRoPE pairs k-blocks
+  P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n);
+  P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes);
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
   P.a_prefetch = (EPI == EPI_CODES) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
   P.msb = P.m_tiles;
@@ -840,7 +848,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
     int msb = (int)std::max<long long>(1, (32ll << 20) / a_tile_bytes);
     if (msb < P.m_tiles) P.msb = msb;
   }
-  const size_t smem = tc_smem_bytes(P.block_n, P.stages);
+  const size_t smem = tc_smem_bytes(P.block_n, P.stages, P.stg_warp_bytes);
   static thread_local size_t configured = 0;   // per instantiation
   if (configured < smem) {
     cudaError_t e = cudaFuncSetAttribute(tc_gemm_kernel<EPI, AMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
