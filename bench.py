@@ -103,6 +103,7 @@ def workload_costs(cfg, T, reuse_rank=None):
     c["gemm2_flops_per_launch"] = T * 2 * d_a * d
     c["gemm3_flops_per_launch"] = T * 2 * d * 2 * D
     c["gemm1_flops_per_launch"] = T * 2 * r * d_a
+    c["gemm1_bytes_per_layer"] = T * (r * cb + sb + d_a * ob)
     return c
 
 
@@ -359,6 +360,13 @@ def run_ours(args, cfg):
             name = {120: "patch_gemm1", 130: "patch_gemm2", 140: "patch_gemm3"}[kid]
             per_layer = costs[{120: "gemm1_flops_per_launch", 130: "gemm2_flops_per_launch", 140: "gemm3_flops_per_launch"}[kid]]
             layers_per_launch = len(cfg.patch_layers) / per_pass
+            if kid == 120:      # K = r is small: the write of the [T, d_a] activation bounds GEMM-1
+                ach = costs["gemm1_bytes_per_layer"] * layers_per_launch / (avg_ms * 1e-3) / 1e9
+                rooflines[name] = {"kernel": KERNEL_NAMES[kid], "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"],
+                                   "unit": "GB/s", "frac": ach / peaks["hbm_gbs"], "traffic": traffic.get(name),
+                                   "ms": avg_ms, "layers_per_launch": layers_per_launch,
+                                   "share_of_step": avg_ms * per_pass / step_ms}
+                continue
             ach = per_layer * layers_per_launch / (avg_ms * 1e-3) / 1e12
             rooflines[name] = {"kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach,
                                "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
