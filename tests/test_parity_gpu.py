@@ -149,6 +149,22 @@ def test_ranks_that_are_not_powers_of_two(rank, cuda_device):
     _run_all(_problem(cfg, cuda_device))
 
 
+def test_all_layers_patch_with_mixed_code_ranks(cuda_device):
+    """L_patch = all layers (legal), with PATCH layers whose r_h differ: scd_patch runs each GEMM stage for a
+    group of consecutive layers of equal (r_h, d_a) as one launch, so ranks 128, 64, 64, 128 exercise groups of 1, 2, 1."""
+    cfg = MINI["llama3_8b_8k"].scaled(seqlens=(333,), n_layers=4, patch_layers=(0, 1, 2, 3), d_model=512)
+    arts = [W.make_layer_artifacts(cfg, l, cuda_device, total_rows=333) for l in range(4)]
+    g = torch.Generator(device=cuda_device).manual_seed(5)
+    for l in (1, 2):                                   # a narrower H code for the two middle layers (random W1: d_a != width of B_H)
+        a = arts[l]
+        a.enc_h = a.enc_h[:, :64].contiguous()
+        a.w1 = (torch.randn(64, cfg.d_a, generator=g, device=cuda_device) / 8.0).to(a.w1.dtype)
+    prob = _problem(cfg, cuda_device, artifacts=arts)
+    assert [prob.plan.code_segment(l, 2, prob.T)[2] for l in range(4)] == [128, 64, 64, 128]
+    res = _run_all(prob)
+    print(res)
+
+
 @pytest.mark.parametrize("state", ["f32", "bf16"])
 def test_edge_batches(state, cuda_device):
     """Ragged lengths that are not multiples of 16 / 128, a 1-token request, position offsets,
