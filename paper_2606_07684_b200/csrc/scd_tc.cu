@@ -39,18 +39,23 @@ struct __align__(8) TcBarriers {
 
 // per-warp staging the epilogue needs: 32 rows x the widest sub-tile row, in whole 128-B swizzle spans.  The encode
 // epilogue (narrow code tiles) needs half of STG_WARP_BYTES; the shared memory it leaves buys a pipeline stage.
+// Shared memory is what buys pipeline stages, and three 48 KB stages (128 x 256 tiles) do not cover the TMA latency of the
+// PATCH GEMM-2 (K = d_a).  Its epilogue is off the critical path, so it stages 64 columns at a time (4 KB per warp) and reads
+// the bias straight from L1/L2 instead of a per-warp shared copy: that is the room for a fourth stage.
+static int tc_sub_n(int epi) { return epi == EPI_U ? 64 : SUB_N; }
+static int tc_vec_warp_bytes(int epi) { return epi == EPI_U ? 0 : VEC_WARP_BYTES; }
 static int tc_stg_warp_bytes(int epi, int block_n) {
-  if (epi != EPI_CODES) return STG_WARP_BYTES;
+  if (epi == EPI_KV) return STG_WARP_BYTES;
   const int cols = (block_n % 64) == 0 ? block_n / 2 : block_n;      // the warp pair splits the columns (gran = 32)
-  const int sub = cols < SUB_N ? cols : SUB_N;
+  const int sub = cols < tc_sub_n(epi) ? cols : tc_sub_n(epi);
   return 32 * ((sub * 2 + 127) & ~127);
 }
-static size_t tc_smem_bytes(int block_n, int stages, int stg_warp_bytes) {
+static size_t tc_smem_bytes(int block_n, int stages, int stg_warp_bytes, int vec_warp_bytes) {
   return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) +
-         EPI_WARPS * (stg_warp_bytes + VEC_WARP_BYTES) + sizeof(TcBarriers);
+         EPI_WARPS * (stg_warp_bytes + vec_warp_bytes) + sizeof(TcBarriers);
 }
-static int tc_pick_stages(int block_n, int num_kb, int stg_warp_bytes) {
-  const size_t budget = 232448 - 1024 - EPI_WARPS * (stg_warp_bytes + VEC_WARP_BYTES) - sizeof(TcBarriers);
+static int tc_pick_stages(int block_n, int num_kb, int stg_warp_bytes, int vec_warp_bytes) {
+  const size_t budget = 232448 - 1024 - EPI_WARPS * (stg_warp_bytes + vec_warp_bytes) - sizeof(TcBarriers);
   int st = (int)(budget / (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2));
   st = st > MAX_STAGES ? MAX_STAGES : st;
   if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty
@@ -208,7 +213,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
   uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
   uint8_t* smem_vec = smem_stg + EPI_WARPS * P.stg_warp_bytes;
-  TcBarriers* bars = (TcBarriers*)(smem_vec + EPI_WARPS * VEC_WARP_BYTES);
+  constexpr bool VEC_SMEM = EPI != EPI_U;   // else the bias is read through L1 (tc_vec_warp_bytes)
+  TcBarriers* bars = (TcBarriers*)(smem_vec + (VEC_SMEM ? EPI_WARPS * VEC_WARP_BYTES : 0));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.n_segs * P.n_tiles * P.m_tiles;
@@ -395,10 +401,12 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // this warp's copy of the tile's mean / bias slice: wvec[c] for tile column c
       __syncwarp();
+      if (VEC_SMEM) {
       asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(cur.m0.x), "f"(cur.m0.y),
                    "f"(cur.m0.z), "f"(cur.m0.w) : "memory");
       asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + 512 + lane * 16), "f"(cur.m1.x), "f"(cur.m1.y),
                    "f"(cur.m1.z), "f"(cur.m1.w) : "memory");
+      }
       __syncwarp();
 
       ptx::mbar_wait_suspend(&bars->tmem_full[acc], acc_phase);
@@ -452,11 +460,11 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         cur = nxt;
         continue;
       }
-      for (int c0 = g_begin; c0 < g_end; c0 += SUB_N) {
-        const int sub_cols = min(SUB_N, g_begin + grp_cols - c0);
+      for (int c0 = g_begin; c0 < g_end; c0 += P.sub_n) {
+        const int sub_cols = min(P.sub_n, g_begin + grp_cols - c0);
         const int row_bytes = sub_cols * out_eb;
         const int pitch = (row_bytes + 127) & ~127;            // whole 128-B swizzle spans
-        const bool last_sub = c0 + SUB_N >= g_end;
+        const bool last_sub = c0 + P.sub_n >= g_end;
 
         if (EPI == EPI_KV && (n0 + c0) < sg.rope_cols && P.rope_style == SCD_ROPE_HALF) {
           // ---- RoPE, HALF pairing (generic): heads of this sub-tile, 16 pairs at a time ----
@@ -501,7 +509,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
             float v[32];
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-              const float4 m4 = ptx::lds_f4(wvec + (c + q * 4) * 4);
+              const float4 m4 = VEC_SMEM ? ptx::lds_f4(wvec + (c + q * 4) * 4)
+                                         : (sg.col_vec ? ldg_f4(sg.col_vec + n0 + c + q * 4) : make_float4(0.f, 0.f, 0.f, 0.f));
               if (EPI == EPI_CODES) {
                 v[q * 4] = __uint_as_float(r[q * 4]) - m4.x; v[q * 4 + 1] = __uint_as_float(r[q * 4 + 1]) - m4.y;
                 v[q * 4 + 2] = __uint_as_float(r[q * 4 + 2]) - m4.z; v[q * 4 + 3] = __uint_as_float(r[q * 4 + 3]) - m4.w;
@@ -838,8 +847,9 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.num_kb = (P.K + BLOCK_K - 1) / BLOCK_K;
   const int total = P.n_segs * P.m_tiles * P.n_tiles;
   if (total <= 0) return SCD_OK;
+  P.sub_n = tc_sub_n(EPI);
   P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n);
-  P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes);
+  P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI));
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
   P.a_prefetch = (EPI == EPI_CODES) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
   P.msb = P.m_tiles;
@@ -848,7 +858,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
     int msb = (int)std::max<long long>(1, (32ll << 20) / a_tile_bytes);
     if (msb < P.m_tiles) P.msb = msb;
   }
-  const size_t smem = tc_smem_bytes(P.block_n, P.stages, P.stg_warp_bytes);
+  const size_t smem = tc_smem_bytes(P.block_n, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI));
   static thread_local size_t configured = 0;   // per instantiation
   if (configured < smem) {
     cudaError_t e = cudaFuncSetAttribute(tc_gemm_kernel<EPI, AMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
