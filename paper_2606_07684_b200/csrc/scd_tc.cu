@@ -42,12 +42,13 @@ struct __align__(8) TcBarriers {
 // Shared memory is what buys pipeline stages, and three 48 KB stages (128 x 256 tiles) do not cover the TMA latency of the
 // PATCH GEMM-2 (K = d_a).  Its epilogue is off the critical path, so it stages 64 columns at a time (4 KB per warp) and reads
 // the bias straight from L1/L2 instead of a per-warp shared copy: that is the room for a fourth stage.
-static int tc_sub_n(int epi) { return epi == EPI_U ? 64 : SUB_N; }
-static int tc_vec_warp_bytes(int epi) { return epi == EPI_U ? 0 : VEC_WARP_BYTES; }
-static int tc_stg_warp_bytes(int epi, int block_n) {
+static int tc_sub_n(int epi, bool compact) { return (epi == EPI_U || compact) ? 64 : SUB_N; }
+static int tc_vec_warp_bytes(int epi, bool compact) { return (epi == EPI_U || compact) ? 0 : VEC_WARP_BYTES; }
+static int tc_stg_warp_bytes(int epi, int block_n, bool compact) {
+  if (compact) return 32 * 128;
   if (epi == EPI_KV) return STG_WARP_BYTES;
   const int cols = (block_n % 64) == 0 ? block_n / 2 : block_n;      // the warp pair splits the columns (gran = 32)
-  const int sub = cols < tc_sub_n(epi) ? cols : tc_sub_n(epi);
+  const int sub = cols < tc_sub_n(epi, false) ? cols : tc_sub_n(epi, false);
   return 32 * ((sub * 2 + 127) & ~127);
 }
 static size_t tc_smem_bytes(int block_n, int stages, int stg_warp_bytes, int vec_warp_bytes) {
@@ -184,6 +185,70 @@ __device__ __forceinline__ void rope_tile_h128(const TcParams& P, uint32_t t_row
     }
   }
 }
+// Compact variant for long-K tiles (PATCH GEMM-3), where the epilogue is off the critical path and shared memory is
+// better spent on a fourth pipeline stage: one head at a time through a 4 KB per-warp staging tile (row = run a | run b,
+// 64 B each), bias read through L1, (cos, sin) recomputed per head.  `bias` = col_vec + n0 or null.
+template <int JG>
+__device__ __forceinline__ void rope_tile_h128_compact(const TcParams& P, uint32_t t_row, uint32_t stg, const float* bias,
+                                                       int pos, float rs, unsigned long long my_row_ptr, int lane) {
+  const unsigned long long rs2 = f2_pack(rs, rs);
+#pragma unroll 1
+  for (int h = 0; h < 2; ++h) {
+#pragma unroll
+    for (int jj = 0; jj < 32; jj += 16) {
+      unsigned long long c2[8], s2[8], ns2[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const float2 x = rope_cs(pos, P.rope_g[JG * 32 + jj + 2 * i]), y = rope_cs(pos, P.rope_g[JG * 32 + jj + 2 * i + 1]);
+        c2[i] = f2_pack(x.x, y.x);
+        s2[i] = f2_pack(x.y, y.y);
+        ns2[i] = f2_pack(-x.y, -y.y);
+      }
+      uint32_t ra[16], rb[16];
+      const int ca = h * 128 + JG * 32 + jj;          // tile column of the "a" elements; "b" = +64
+      ptx::tmem_ld16(t_row + ca, ra);
+      ptx::tmem_ld16(t_row + ca + 64, rb);
+      ptx::tmem_ld_wait();
+      uint32_t oa[8], ob[8];
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        const float4 ma = bias ? ldg_f4(bias + ca + q * 4) : z4, mb = bias ? ldg_f4(bias + ca + 64 + q * 4) : z4;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          const int i = q * 4 + e * 2;
+          const unsigned long long a = f2_fma(f2_pack(__uint_as_float(ra[i]), __uint_as_float(ra[i + 1])), rs2,
+                                              e ? f2_pack(ma.z, ma.w) : f2_pack(ma.x, ma.y));
+          const unsigned long long b = f2_fma(f2_pack(__uint_as_float(rb[i]), __uint_as_float(rb[i + 1])), rs2,
+                                              e ? f2_pack(mb.z, mb.w) : f2_pack(mb.x, mb.y));
+          float x0, x1, y0, y1;
+          f2_unpack(f2_fma(b, ns2[i >> 1], f2_mul(a, c2[i >> 1])), x0, x1);   // a cos - b sin
+          f2_unpack(f2_fma(a, s2[i >> 1], f2_mul(b, c2[i >> 1])), y0, y1);    // b cos + a sin
+          oa[q * 2 + e] = pack_bf16x2(x0, x1);
+          ob[q * 2 + e] = pack_bf16x2(y0, y1);
+        }
+      }
+      const int k0 = jj >> 3;                          // chunk of run a; run b = +4
+      stg_put(stg, 128, lane, k0, make_uint4(oa[0], oa[1], oa[2], oa[3]));
+      stg_put(stg, 128, lane, k0 + 1, make_uint4(oa[4], oa[5], oa[6], oa[7]));
+      stg_put(stg, 128, lane, k0 + 4, make_uint4(ob[0], ob[1], ob[2], ob[3]));
+      stg_put(stg, 128, lane, k0 + 5, make_uint4(ob[4], ob[5], ob[6], ob[7]));
+    }
+    __syncwarp();
+    {
+      const int l = lane & 7;                          // 8 lanes per row: run l / 4, chunk l % 4
+      const unsigned long long off = (unsigned long long)((h * 128 + (l >> 2) * 64 + JG * 32 + (l & 3) * 8) * 2);
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        const int r = it * 4 + (lane >> 3);
+        const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
+        const uint4 v = ptx::lds128(stg_addr(stg, 128, r, l));
+        if (base != 0ull) ptx::stg128(base + off, v);
+      }
+    }
+    __syncwarp();
+  }
+}
 // copy-out of the 4-run layout above: lane l of a half-warp holds run l / 4, chunk l % 4
 template <int JG>
 __device__ __forceinline__ void rope_tile_h128_copy_out(uint32_t stg, unsigned long long my_row_ptr, int lane) {
@@ -214,7 +279,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
   uint8_t* smem_vec = smem_stg + EPI_WARPS * P.stg_warp_bytes;
   constexpr bool VEC_SMEM = EPI != EPI_U;   // else the bias is read through L1 (tc_vec_warp_bytes)
-  TcBarriers* bars = (TcBarriers*)(smem_vec + (VEC_SMEM ? EPI_WARPS * VEC_WARP_BYTES : 0));
+  const bool vec_smem = VEC_SMEM && !(EPI == EPI_KV && P.kv_compact);
+  TcBarriers* bars = (TcBarriers*)(smem_vec + (vec_smem ? EPI_WARPS * VEC_WARP_BYTES : 0));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.n_segs * P.n_tiles * P.m_tiles;
@@ -401,7 +467,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // this warp's copy of the tile's mean / bias slice: wvec[c] for tile column c
       __syncwarp();
-      if (VEC_SMEM) {
+      if (vec_smem) {
       asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(cur.m0.x), "f"(cur.m0.y),
                    "f"(cur.m0.z), "f"(cur.m0.w) : "memory");
       asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + 512 + lane * 16), "f"(cur.m1.x), "f"(cur.m1.y),
@@ -420,6 +486,16 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       if (EPI == EPI_KV && n0 < sg.rope_cols && P.rope_style == SCD_ROPE_HALF && P.head_dim == 128 && block_n == 256 &&
           n_end == 256) {
         // ---- 2-head K tile: frequency split between the warp pair ----
+        if (P.kv_compact) {
+          const float* bias = sg.col_vec ? sg.col_vec + n0 : nullptr;
+          if (grp == 0) rope_tile_h128_compact<0>(P, t_row, stg, bias, pos, rs, row_ptr, lane);
+          else rope_tile_h128_compact<1>(P, t_row, stg, bias, pos, rs, row_ptr, lane);
+          ptx::tc_fence_before();
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+          cur = nxt;
+          continue;
+        }
         if (grp == 0) rope_tile_h128<0>(P, t_row, stg, wvec, pos, rs, lane);
         else rope_tile_h128<1>(P, t_row, stg, wvec, pos, rs, lane);
         ptx::tc_fence_before();
@@ -509,7 +585,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
             float v[32];
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-              const float4 m4 = VEC_SMEM ? ptx::lds_f4(wvec + (c + q * 4) * 4)
+              const float4 m4 = vec_smem ? ptx::lds_f4(wvec + (c + q * 4) * 4)
                                          : (sg.col_vec ? ldg_f4(sg.col_vec + n0 + c + q * 4) : make_float4(0.f, 0.f, 0.f, 0.f));
               if (EPI == EPI_CODES) {
                 v[q * 4] = __uint_as_float(r[q * 4]) - m4.x; v[q * 4 + 1] = __uint_as_float(r[q * 4 + 1]) - m4.y;
@@ -773,6 +849,9 @@ static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, i
   return SCD_OK;
 }
 
+#ifndef G3_GENERIC
+#define G3_GENERIC 1
+#endif
 #ifndef TC_A_PREFETCH
 #define TC_A_PREFETCH 4
 #endif
@@ -847,9 +926,13 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.num_kb = (P.K + BLOCK_K - 1) / BLOCK_K;
   const int total = P.n_segs * P.m_tiles * P.n_tiles;
   if (total <= 0) return SCD_OK;
-  P.sub_n = tc_sub_n(EPI);
-  P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n);
-  P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI));
+  // compact paged-KV epilogue: long-K tiles of two 128-wide heads (PATCH GEMM-3)
+  const bool compact = EPI == EPI_KV && P.num_kb >= 16 && P.block_n == 256 && P.head_dim == 128 && P.rope_style == SCD_ROPE_HALF &&
+                       (P.N % 256) == 0;
+  P.kv_compact = compact ? 1 : 0;
+  P.sub_n = tc_sub_n(EPI, compact);
+  P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n, compact);
+  P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
   P.a_prefetch = (EPI == EPI_CODES) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
   P.msb = P.m_tiles;
@@ -858,7 +941,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
     int msb = (int)std::max<long long>(1, (32ll << 20) / a_tile_bytes);
     if (msb < P.m_tiles) P.msb = msb;
   }
-  const size_t smem = tc_smem_bytes(P.block_n, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI));
+  const size_t smem = tc_smem_bytes(P.block_n, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
   static thread_local size_t configured = 0;   // per instantiation
   if (configured < smem) {
     cudaError_t e = cudaFuncSetAttribute(tc_gemm_kernel<EPI, AMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -1116,7 +1199,12 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
       sg.b_map = 2 * nseg + 3 * (int)(j0 + q) + 2;
     }
     P.prof_id = SCD_PROF_PATCH_GEMM3;
-    if ((st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK) return st;
+    // long K (d_model >= 1024): the generic kernel with the compact epilogue runs four pipeline stages where the
+    // paged-KV kernel has room for three; short K: the paged-KV kernel's faster epilogue wins
+    const bool long_k = G3_GENERIC && d >= 16 * BLOCK_K;
+    if ((st = (!long_k && tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size)) ? launch_tc_kv(p, P, s)
+                                                                                       : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK)
+      return st;
     j0 = j1;
   }
   return SCD_OK;

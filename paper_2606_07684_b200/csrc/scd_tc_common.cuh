@@ -33,6 +33,7 @@ struct TcParams {
   BatchDev batch;
   int32_t n_segs, M, N, K;
   int32_t m_tiles, n_tiles, num_kb, block_n, stages;
+  int32_t kv_compact;                 // generic kernel, EPI_KV: compact epilogue (4 KB staging, bias through L1)
   int32_t sub_n;                      // generic kernel: columns per epilogue staging sub-tile
   int32_t stg_warp_bytes;             // generic kernel: per-warp epilogue staging bytes
   int32_t a_prefetch;                 // generic kernel: k-blocks of A pulled into L2 ahead of their TMA load (0 = off)
