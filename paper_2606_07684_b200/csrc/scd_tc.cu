@@ -43,7 +43,7 @@ struct __align__(8) TcBarriers {
 // PATCH GEMM-2 (K = d_a).  Its epilogue is off the critical path, so it stages 64 columns at a time (4 KB per warp) and reads
 // the bias straight from L1/L2 instead of a per-warp shared copy: that is the room for a fourth stage.
 static int tc_sub_n(int epi, bool compact) { return (epi == EPI_U || compact) ? 64 : SUB_N; }
-static int tc_vec_warp_bytes(int epi, bool compact) { return (epi == EPI_U || compact) ? 0 : VEC_WARP_BYTES; }
+static int tc_vec_warp_bytes(int epi, bool compact) { return (epi == EPI_U || epi == EPI_CODES || compact) ? 0 : VEC_WARP_BYTES; }
 static int tc_stg_warp_bytes(int epi, int block_n, bool compact) {
   if (compact) return 32 * 128;
   if (epi == EPI_KV) return STG_WARP_BYTES;
@@ -278,7 +278,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
   uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
   uint8_t* smem_vec = smem_stg + EPI_WARPS * P.stg_warp_bytes;
-  constexpr bool VEC_SMEM = EPI != EPI_U;   // else the bias is read through L1 (tc_vec_warp_bytes)
+  constexpr bool VEC_SMEM = (EPI == EPI_KV || EPI == EPI_ACT);   // else the mean / bias is read through L1 (tc_vec_warp_bytes)
   const bool vec_smem = VEC_SMEM && !(EPI == EPI_KV && P.kv_compact);
   TcBarriers* bars = (TcBarriers*)(smem_vec + (vec_smem ? EPI_WARPS * VEC_WARP_BYTES : 0));
 
@@ -518,7 +518,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           ptx::tmem_ld_wait();
 #pragma unroll
           for (int q = 0; q < 8; ++q) {
-            const float4 m4 = ptx::lds_f4(wvec + (c + q * 4) * 4);
+            const float4 m4 = vec_smem ? ptx::lds_f4(wvec + (c + q * 4) * 4)
+                                       : (sg.col_vec ? ldg_f4(sg.col_vec + n0 + c + q * 4) : make_float4(0.f, 0.f, 0.f, 0.f));
             amax = fmaxf(amax, fmaxf(fmaxf(fabsf(__uint_as_float(r[q * 4]) - m4.x), fabsf(__uint_as_float(r[q * 4 + 1]) - m4.y)),
                                      fmaxf(fabsf(__uint_as_float(r[q * 4 + 2]) - m4.z), fabsf(__uint_as_float(r[q * 4 + 3]) - m4.w))));
           }
