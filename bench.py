@@ -369,8 +369,11 @@ def run_ours(args, cfg):
                 continue
             ach = per_layer * layers_per_launch / (avg_ms * 1e-3) / 1e12
             rooflines[name] = {"kernel": KERNEL_NAMES[kid], "bound": "tensor", "achieved": ach,
-                               "peak": peaks["bf16_tflops_sustained"], "unit": "TFLOP/s",
-                               "frac": ach / peaks["bf16_tflops_sustained"], "traffic": traffic.get(name), "ms": avg_ms,
+                               # each launch is timed on its own (events around it, a 0.3-0.6 ms kernel after an L2
+                               # flush): the burst figure is the peak that applies; the sustained one is reported beside it
+                               "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                               "frac": ach / peaks["bf16_tflops"], "frac_of_sustained_peak": ach / peaks["bf16_tflops_sustained"],
+                               "traffic": traffic.get(name), "ms": avg_ms,
                                "layers_per_launch": layers_per_launch, "share_of_step": avg_ms * per_pass / step_ms}
         elif kid in (100, 101):
             pass
@@ -383,7 +386,7 @@ def run_ours(args, cfg):
     roofline = dict(rooflines[dom_key]) if dom_key else None
     if roofline:
         roofline["name"] = dom_key
-        roofline["peak_source"] = peaks["source"] + (" sustained bf16" if roofline["bound"] == "tensor" else " copy")
+        roofline["peak_source"] = peaks["source"] + (" burst bf16 (kernel timed alone)" if roofline["bound"] == "tensor" else " copy")
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
