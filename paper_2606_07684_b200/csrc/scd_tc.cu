@@ -4,20 +4,23 @@
 // K-major, plus an A-side transform and a fused epilogue (scd_internal.h: EpiKind, AMode).
 // One persistent, warp-specialised kernel template serves all of them:
 //
-//   warp 0      TMA producer: A tile [128 x 64] and Bt tile [BLOCK_N x 64] per k-block into a
-//               4-deep shared-memory ring (128-byte swizzle), mbarrier expect_tx / complete_tx
-//   warp 1      MMA issuer: one elected thread issues tcgen05.mma (128 x BLOCK_N x 16, bf16 ->
-//               fp32) into one of two TMEM accumulator buffers; tcgen05.commit releases the
-//               smem stage and finally signals the epilogue
-//   warp 2      TMEM allocator (512 columns = 2 accumulator buffers of <= 256 columns)
-//   warps 4-7   epilogue: tcgen05.ld (one token row per thread), fused mean / row-scale /
-//               RoPE / activation / quantisation, 16-byte stores (codes, workspace, or the
-//               token's slot of the paged KV pool); overlaps the next tile's MMAs
-//   warps 8-11  (A_DEROPE only) rotate the freshly landed K tile in shared memory by
-//               -position (Eq. 5) before the MMA may read it
+//   warp 0        TMA producer: A tile [128 x 64] and Bt tile [BLOCK_N x 64] per k-block into a shared-memory
+//                 ring (128-byte swizzle, 3-6 stages: as many as the launch's epilogue leaves room for),
+//                 mbarrier expect_tx / complete_tx; the encode's A stream is pulled into L2 a few k-blocks ahead
+//   warp 1        MMA issuer: one elected thread issues tcgen05.mma (128 x BLOCK_N x 16, bf16 -> fp32) into one
+//                 of two TMEM accumulator buffers; tcgen05.commit releases the smem stage and finally signals
+//                 the epilogue
+//   warp 2        TMEM allocator (512 columns = 2 accumulator buffers of 256 columns)
+//   warps 4-11    epilogue: tcgen05.ld (one token row per thread; the two warps of a lane quadrant split the
+//                 columns or, for two-head K tiles, the RoPE frequencies), fused mean / row-scale / RoPE /
+//                 activation / quantisation, swizzled per-warp staging, coalesced 16-byte stores (codes,
+//                 workspace, or the token's slot of the paged KV pool); overlaps the next tile's MMAs
+//   warps 12-27   (A_DEROPE / A_CODES only) transform the freshly landed A tile in shared memory, 4 threads per
+//                 token row, before the MMA may read it: rotate K by -position (Eq. 5) / widen e4m3 codes to bf16
 //
-// A launch covers many (layer, branch) segments of equal shape: tile -> (segment, n-tile,
-// m-tile) with m fastest, tiles dealt round-robin to one CTA per SM.
+// A launch covers many (layer, branch) segments of equal shape: tile -> (segment, L2 super-block, n-tile,
+// m-tile) with m fastest, tiles dealt round-robin to one CTA per SM.  Launched with programmatic stream
+// serialisation: everything above the first global access overlaps the previous kernel's tail.
 #include <algorithm>
 #include <cmath>
 #include <cstring>

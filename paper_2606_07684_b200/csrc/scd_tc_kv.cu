@@ -1,5 +1,6 @@
-// Paged-KV specialisation of the tcgen05 GEMM: REUSE decode (Eq. 9) and PATCH
-// GEMM-3 (Eq. 12a/b) for head_dim 128, HALF RoPE, 256-column (two-head) tiles.
+// Paged-KV specialisation of the tcgen05 GEMM: REUSE decode (Eq. 9) and short-K PATCH
+// GEMM-3 (Eq. 12a/b) for head_dim 128, HALF RoPE, 256-column (two-head) tiles.  (Long-K GEMM-3
+// runs on scd_tc.cu's kernel with its compact epilogue, which leaves room for a fourth pipeline stage.)
 //
 // Same TMA -> tcgen05 -> TMEM main loop as scd_tc.cu; what differs is the tile order and the epilogue,
 // which is where this kernel's time goes (it writes 8x what it reads):
