@@ -82,6 +82,27 @@ def test_code_layout_matches_oracle_payload(B, code):
     assert B.scd_code_layout(model, layers, 0)[3] == 0
 
 
+def test_code_layout_per_head_reading(B):
+    """reuse_per_head: r_k / r_v are per-head ranks, a token's code row is H * r wide; the
+    library's layout and payload agree with the oracle's accounting, PATCH segments are unaffected, and the
+    16-byte row-pitch rule applies to the effective width."""
+    kinds = [B.SCD_REUSE, B.SCD_PATCH, B.SCD_REUSE]
+    model, layers = _descs(B, kinds, r_k=12, r_v=4, r_h=32)          # H = 2: code rows 24 and 8 wide
+    model.reuse_per_head = 1
+    T = 777
+    ol = [O.Layer(O.REUSE, enc_k=np.zeros((64, 12)), enc_v=np.zeros((64, 4))) if k == B.SCD_REUSE
+          else O.Layer(O.PATCH, enc_h=np.zeros((1, 32))) for k in kinds]
+    om = O.Model(n_layers=3, d_model=512, n_kv_heads=2, head_dim=64, code_dtype=B.SCD_BF16, reuse_per_head=True)
+    _, _, _, code_bytes, payload = B.scd_code_layout(model, layers, T)
+    assert payload == O.payload_bytes(om, ol, T) == T * 2 * (2 * 24 + 2 * 8 + 32)
+    assert B.scd_code_layout(model, layers, T, 0, 0)[2] == 24 and B.scd_code_layout(model, layers, T, 2, 1)[2] == 8
+    assert B.scd_code_layout(model, layers, T, 1, 2)[2] == 32
+    layers[0].r_k = 2                                                # H * r = 4: not a multiple of 8 on the bf16 path
+    with pytest.raises(B.ScdError) as e:
+        B.scd_code_layout(model, layers, T)
+    assert e.value.status == 3
+
+
 def test_host_side_validation(B):
     model, layers = _descs(B, [B.SCD_REUSE, B.SCD_PATCH])
     arr = (B.LayerDesc * 2)(*layers)
