@@ -165,6 +165,27 @@ def test_all_layers_patch_with_mixed_code_ranks(cuda_device):
     print(res)
 
 
+@pytest.mark.parametrize("seed", range(6))
+def test_random_ragged_batches(seed, cuda_device):
+    """Seeded random draws over what the tests above fix by hand (tier 4): request count and lengths (1 ... 700,
+    so tiles straddle requests and pages are partial), permuted pages, position offsets, the PATCH set (empty, some, all),
+    rank, per-head vs per-layer REUSE, bf16 vs e4m3 codes."""
+    rng = np.random.default_rng(1000 + seed)
+    n_layers = int(rng.integers(1, 5))
+    patch = tuple(int(l) for l in range(n_layers) if rng.random() < 0.4)
+    seqlens = tuple(int(x) for x in rng.integers(1, 700, int(rng.integers(1, 6))))
+    e4 = bool(rng.random() < 0.35)
+    base = MINI["mistral_7b_32k_fp8"] if e4 else MINI["llama3_8b_8k"]
+    per_head = 0 if rng.random() < 0.6 else int(rng.choice([16, 32]))
+    rank = int(rng.choice([64, 128, 256] if e4 else [32, 64, 96, 128, 256]))
+    cfg = base.scaled(n_layers=n_layers, patch_layers=patch, seqlens=seqlens, ragged_range=None, permute_pages=True,
+                      d_model=int(rng.choice([512, 1024])), rank=rank)
+    offs = [int(x) for x in rng.integers(0, 3000, len(seqlens))]
+    prob = _problem(cfg, cuda_device, pos_offset=offs, per_head_rank=per_head)
+    res = _run_all(prob)
+    print(seed, n_layers, patch, seqlens, rank, per_head, "e4m3" if e4 else "bf16", res)
+
+
 @pytest.mark.parametrize("state", ["f32", "bf16"])
 def test_edge_batches(state, cuda_device):
     """Ragged lengths that are not multiples of 16 / 128, a 1-token request, position offsets,
