@@ -109,9 +109,11 @@ __device__ __forceinline__ void stg_put(uint32_t stg, int pitch, int row, int ch
 // Copy the warp's staged sub-tile (32 rows x row_bytes) to global: LPR lanes cover one row with
 // one fully coalesced 16-B store each; row base pointers come from the owning lane by shuffle
 // (null = row beyond M).  `valid_bytes` masks the N tail.
+// `streaming`: pool rows and codes are written once and not read back by this call chain -> evict-first stores, so
+// they do not push the operands out of L2; workspace tensors (read by the next GEMM) use plain stores.
 template <int LPR>
 __device__ __forceinline__ void stg_copy_out_t(uint32_t stg, int pitch, int valid_bytes, unsigned long long my_row_ptr,
-                                               unsigned long long byte_off, int lane) {
+                                               unsigned long long byte_off, int lane, bool streaming) {
   constexpr int rpi = 32 / LPR;
   const int chunk = lane % LPR;
 #pragma unroll
@@ -119,19 +121,22 @@ __device__ __forceinline__ void stg_copy_out_t(uint32_t stg, int pitch, int vali
     const int r = it * rpi + lane / LPR;
     const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
     const uint4 v = ptx::lds128(stg_addr(stg, pitch, r, chunk));
-    if (base != 0ull && chunk * 16 < valid_bytes) ptx::stg128(base + byte_off + (unsigned long long)chunk * 16, v);
+    if (base != 0ull && chunk * 16 < valid_bytes) {
+      if (streaming) ptx::stg128_cs(base + byte_off + (unsigned long long)chunk * 16, v);
+      else ptx::stg128(base + byte_off + (unsigned long long)chunk * 16, v);
+    }
   }
 }
 __device__ __forceinline__ void stg_copy_out(uint32_t stg, int pitch, int row_bytes, int valid_bytes,
-                                             unsigned long long my_row_ptr, unsigned long long byte_off, int lane) {
+                                             unsigned long long my_row_ptr, unsigned long long byte_off, int lane, bool streaming) {
   int lpr = 1;
   while (lpr * 16 < row_bytes) lpr <<= 1;             // lanes per row: next power of two
   switch (lpr) {
-    case 16: stg_copy_out_t<16>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
-    case 8: stg_copy_out_t<8>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
-    case 4: stg_copy_out_t<4>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
-    case 2: stg_copy_out_t<2>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
-    default: stg_copy_out_t<1>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane); break;
+    case 16: stg_copy_out_t<16>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane, streaming); break;
+    case 8: stg_copy_out_t<8>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane, streaming); break;
+    case 4: stg_copy_out_t<4>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane, streaming); break;
+    case 2: stg_copy_out_t<2>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane, streaming); break;
+    default: stg_copy_out_t<1>(stg, pitch, valid_bytes, my_row_ptr, byte_off, lane, streaming); break;
   }
 }
 
@@ -246,7 +251,7 @@ __device__ __forceinline__ void rope_tile_h128_compact(const TcParams& P, uint32
         const int r = it * 4 + (lane >> 3);
         const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
         const uint4 v = ptx::lds128(stg_addr(stg, 128, r, l));
-        if (base != 0ull) ptx::stg128(base + off, v);
+        if (base != 0ull) ptx::stg128_cs(base + off, v);
       }
     }
     __syncwarp();
@@ -262,7 +267,7 @@ __device__ __forceinline__ void rope_tile_h128_copy_out(uint32_t stg, unsigned l
     const int r = it * 2 + (lane >> 4);
     const unsigned long long base = __shfl_sync(0xffffffffu, my_row_ptr, r);
     const uint4 v = ptx::lds128(stg_addr(stg, 256, r, l));
-    if (base != 0ull) ptx::stg128(base + off, v);
+    if (base != 0ull) ptx::stg128_cs(base + off, v);
   }
 }
 
@@ -656,7 +661,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         }
         // valid bytes: the N tail, and never more than this warp staged (a 96-column group rounds its lanes-per-row
         // up to 16 chunks; the 4 extra chunks are the other group's columns)
-        stg_copy_out(stg, pitch, row_bytes, min(row_bytes, (n_end - c0) * out_eb), row_ptr, (unsigned long long)c0 * out_eb, lane);
+        stg_copy_out(stg, pitch, row_bytes, min(row_bytes, (n_end - c0) * out_eb), row_ptr, (unsigned long long)c0 * out_eb, lane,
+                     EPI == EPI_KV || EPI == EPI_CODES);
         __syncwarp();
       }
       if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = ss_u;

@@ -460,7 +460,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          if (base[i] != 0ull) ptx::stg128(base[i] + (unsigned long long)lane * 16ull, v[i]);
+          if (base[i] != 0ull) ptx::stg128_cs(base[i] + (unsigned long long)lane * 16ull, v[i]);
       }
       cur = nxt;
       tc = tn;
