@@ -145,8 +145,9 @@ scd_status_t scd_plan(const scd_model_desc_t* model, const scd_layer_desc_t* lay
 scd_status_t scd_plan_destroy(scd_plan_t* plan);
 
 /* Sizes for a call over `total_tokens` packed rows: code buffer bytes (with padding),
- * workspace bytes scd_patch needs, and the transport payload |Z| of Eq. 3 (
- * codes + e4m3 scales, no padding).  Any out pointer may be NULL. */
+ * the workspace scd_patch prefers (the intermediates of as many PATCH layers as it runs
+ * per launch: up to 2 GiB, never more than all of them), and the transport payload |Z| of
+ * Eq. 3 (codes + e4m3 scales, no padding).  Any out pointer may be NULL. */
 scd_status_t scd_plan_query(const scd_plan_t* plan, int32_t total_tokens,
                             size_t* code_bytes, size_t* patch_workspace_bytes, size_t* payload_bytes);
 
@@ -177,7 +178,10 @@ scd_status_t scd_reuse_decode(const scd_plan_t* plan, const scd_batch_t* batch, 
                               const scd_paged_kv_t* kv, void* stream);
 
 /* Consumer side, PATCH layers only (Eq. 11-12): aligner -> RMS-consistent scaling ->
- * [W_k | W_v] -> RoPE on K -> paged write.  `workspace` >= patch_workspace_bytes. */
+ * [W_k | W_v] -> RoPE on K -> paged write.  `workspace` (DEVICE, 128-byte aligned, caller
+ * owned, contents undefined afterwards): patch_workspace_bytes of scd_plan_query is the
+ * preferred size; anything that holds one PATCH layer's intermediates is accepted (fewer
+ * layers per launch), less returns SCD_E_WORKSPACE before anything is enqueued. */
 scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
                        const scd_paged_kv_t* kv, void* workspace, size_t workspace_bytes, void* stream);
 

@@ -632,9 +632,14 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
   if ((st = check_pools(plan, kv, SCD_PATCH)) != SCD_OK) return st;
   const scd_model_desc_t& m = plan->model;
   const int T = batch->total_tokens;
-  const size_t need = patch_workspace(plan, T);
-  if (!workspace || workspace_bytes < need)
-    return fail(SCD_E_WORKSPACE, "scd_patch needs %zu workspace bytes, got %zu", need, workspace_bytes);
+  // scd_plan_query reports the workspace for the preferred group of layers per launch; any workspace that holds at
+  // least one layer's intermediates is accepted, and the group shrinks to what it holds
+  PatchWs pw = patch_ws(plan, T);
+  const size_t per_layer = pw.act_stride + pw.u_stride + pw.ss_stride;
+  if (pw.group > 0 && (!workspace || workspace_bytes < per_layer))
+    return fail(SCD_E_WORKSPACE, "scd_patch needs at least %zu workspace bytes (%zu preferred), got %zu", per_layer, pw.total(),
+                workspace_bytes);
+  if (pw.group > 0 && (size_t)pw.group * per_layer > workspace_bytes) pw.group = (int)(workspace_bytes / per_layer);
   if (!aligned(workspace, 128)) return fail(SCD_E_ALIGN, "workspace must be 128-byte aligned");
   Layout lay;
   plan_layout(plan, T, &lay);
@@ -643,7 +648,6 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
   int d_a_max = 0;
   for (auto& pp : plan->patches) d_a_max = pp.d_a > d_a_max ? pp.d_a : d_a_max;
   const int d = m.d_model, D = plan->D;
-  const PatchWs pw = patch_ws(plan, T);
   char* ws_act = (char*)workspace;
   char* ws_u = ws_act + (size_t)pw.group * pw.act_stride;
   float* ws_ss = (float*)(ws_u + (size_t)pw.group * pw.u_stride);

@@ -186,6 +186,30 @@ def test_random_ragged_batches(seed, cuda_device):
     print(seed, n_layers, patch, seqlens, rank, per_head, "e4m3" if e4 else "bf16", res)
 
 
+def test_patch_with_a_one_layer_workspace(cuda_device):
+    """scd_patch prefers a workspace for a whole group of PATCH layers (one launch per GEMM stage and group) but must
+    accept one that holds a single layer's intermediates, and produce the same bits."""
+    from paper_2606_07684_b200 import binding as B
+    cfg = MINI["llama3_8b_8k"].scaled(seqlens=(400,), n_layers=3, patch_layers=(0, 1, 2), d_model=512)
+    prob = _problem(cfg, cuda_device)
+    k, v, h = prob.make_sources()
+    prob.alloc_pools()
+    prob.encode(k, v, h)
+    n_full = prob.patch()
+    torch.cuda.synchronize()
+    want = [(kp.clone(), vp.clone()) for kp, vp in zip(prob.k_pool, prob.v_pool)]
+    prob.alloc_pools()
+    one = prob.ws_bytes // 3
+    assert one % 128 == 0
+    n_one = B.scd_patch(prob.plan, prob.bdesc, prob.codes, prob.k_pool, prob.v_pool, prob.batch.n_blocks,
+                        prob.workspace[:one])
+    torch.cuda.synchronize()
+    assert n_full == 3 and n_one == 9                   # 3 stages x 1 group  vs  3 stages x 3 groups of one layer
+    for (kw, vw), kp, vp in zip(want, prob.k_pool, prob.v_pool):
+        assert torch.equal(kw.view(torch.int16), kp.view(torch.int16)) and torch.equal(vw.view(torch.int16), vp.view(torch.int16))
+    P.check_patch(prob)
+
+
 @pytest.mark.parametrize("state", ["f32", "bf16"])
 def test_edge_batches(state, cuda_device):
     """Ragged lengths that are not multiples of 16 / 128, a 1-token request, position offsets,
