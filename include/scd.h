@@ -185,6 +185,23 @@ scd_status_t scd_reuse_decode(const scd_plan_t* plan, const scd_batch_t* batch, 
 scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
                        const scd_paged_kv_t* kv, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Layer-streamed variants: the same three calls restricted to layers [layer_begin, layer_end)
+ * (0 <= begin <= end <= n_layers, else SCD_E_ARG).  Code segments are per (layer, branch)
+ * (scd_plan_code_segment), so a producer can encode a group of layers, hand their segments
+ * to the transport, and go on with the next group while the consumer decodes / patches the
+ * groups that have arrived: the three terms of Eq. 3 pipelined instead of
+ * summed.  Source states, code segments and pools of layers outside the window are neither
+ * read, written nor validated (their pointers may be NULL); a window without REUSE (PATCH)
+ * layers makes scd_reuse_decode_layers (scd_patch_layers) a no-op returning SCD_OK. */
+scd_status_t scd_encode_layers(const scd_plan_t* plan, const scd_batch_t* batch, const scd_src_t* src,
+                               void* codes, int32_t layer_begin, int32_t layer_end, void* stream);
+scd_status_t scd_reuse_decode_layers(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
+                                     const scd_paged_kv_t* kv, int32_t layer_begin, int32_t layer_end,
+                                     void* stream);
+scd_status_t scd_patch_layers(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
+                              const scd_paged_kv_t* kv, void* workspace, size_t workspace_bytes,
+                              int32_t layer_begin, int32_t layer_end, void* stream);
+
 /* Number of kernels the last hot call on this thread enqueued (for bench accounting). */
 int32_t scd_last_launch_count(void);
 

@@ -31,7 +31,8 @@ NO_SCALE = C.c_size_t(-1).value
 
 # every symbol include/scd.h declares
 EXPORTS = ["scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
-           "scd_encode", "scd_reuse_decode", "scd_patch", "scd_last_launch_count", "scd_profile_enable",
+           "scd_encode", "scd_reuse_decode", "scd_patch", "scd_encode_layers", "scd_reuse_decode_layers",
+           "scd_patch_layers", "scd_last_launch_count", "scd_profile_enable",
            "scd_profile_fetch", "scd_last_error", "scd_version"]
 
 
@@ -92,6 +93,9 @@ def _load() -> C.CDLL:
     lib.scd_encode.argtypes = [vp, C.POINTER(BatchDesc), C.POINTER(SrcDesc), vp, vp]
     lib.scd_reuse_decode.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), vp]
     lib.scd_patch.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), vp, sz, vp]
+    lib.scd_encode_layers.argtypes = [vp, C.POINTER(BatchDesc), C.POINTER(SrcDesc), vp, i32, i32, vp]
+    lib.scd_reuse_decode_layers.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), i32, i32, vp]
+    lib.scd_patch_layers.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), vp, sz, i32, i32, vp]
     for name in ("scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
                  "scd_encode", "scd_reuse_decode", "scd_patch"):
         getattr(lib, name).restype = C.c_int
@@ -223,26 +227,39 @@ def scd_plan(model: ModelDesc, layers: Sequence[LayerDesc], stream=None) -> Plan
 
 def scd_encode(plan: Plan, batch: BatchDesc, k: Sequence[Optional[torch.Tensor]],
                v: Sequence[Optional[torch.Tensor]], h: Sequence[Optional[torch.Tensor]], codes: torch.Tensor,
-               kv_token_stride: int, kv_head_stride: int, h_token_stride: int, stream=None) -> int:
+               kv_token_stride: int, kv_head_stride: int, h_token_stride: int, stream=None, layers=None) -> int:
+    """`layers` = (begin, end): the layer-streamed variant scd_encode_layers."""
     src = SrcDesc(_ptr_array(k), _ptr_array(v), _ptr_array(h), kv_token_stride, kv_head_stride, h_token_stride)
-    _check(lib.scd_encode(plan.handle, C.byref(batch), C.byref(src), _ptr(codes), _stream_ptr(stream)))
+    if layers is None:
+        _check(lib.scd_encode(plan.handle, C.byref(batch), C.byref(src), _ptr(codes), _stream_ptr(stream)))
+    else:
+        _check(lib.scd_encode_layers(plan.handle, C.byref(batch), C.byref(src), _ptr(codes), layers[0], layers[1],
+                                     _stream_ptr(stream)))
     return lib.scd_last_launch_count()
 
 
 def scd_reuse_decode(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequence[Optional[torch.Tensor]],
-                     v_pool: Sequence[Optional[torch.Tensor]], n_blocks: int, stream=None) -> int:
+                     v_pool: Sequence[Optional[torch.Tensor]], n_blocks: int, stream=None, layers=None) -> int:
     kv = PagedKV(_ptr_array(k_pool), _ptr_array(v_pool), n_blocks)
-    _check(lib.scd_reuse_decode(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _stream_ptr(stream)))
+    if layers is None:
+        _check(lib.scd_reuse_decode(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _stream_ptr(stream)))
+    else:
+        _check(lib.scd_reuse_decode_layers(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), layers[0], layers[1],
+                                           _stream_ptr(stream)))
     return lib.scd_last_launch_count()
 
 
 def scd_patch(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequence[Optional[torch.Tensor]],
               v_pool: Sequence[Optional[torch.Tensor]], n_blocks: int, workspace: Optional[torch.Tensor],
-              stream=None) -> int:
+              stream=None, layers=None) -> int:
     kv = PagedKV(_ptr_array(k_pool), _ptr_array(v_pool), n_blocks)
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
-    _check(lib.scd_patch(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _ptr(workspace), ws_bytes,
-                         _stream_ptr(stream)))
+    if layers is None:
+        _check(lib.scd_patch(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _ptr(workspace), ws_bytes,
+                             _stream_ptr(stream)))
+    else:
+        _check(lib.scd_patch_layers(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _ptr(workspace), ws_bytes,
+                                    layers[0], layers[1], _stream_ptr(stream)))
     return lib.scd_last_launch_count()
 
 

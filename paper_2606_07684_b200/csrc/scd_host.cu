@@ -23,6 +23,12 @@ scd_status_t fail(scd_status_t st, const char* fmt, ...) {
   return st;
 }
 void count_launch() { ++g_launches; }
+static thread_local int g_layer_begin = 0, g_layer_end = 1 << 30;
+bool layer_in_window(int layer) { return layer >= g_layer_begin && layer < g_layer_end; }
+struct LayerWindow {                       // scoped: set by the *_layers entry points
+  LayerWindow(int b, int e) { g_layer_begin = b; g_layer_end = e; }
+  ~LayerWindow() { g_layer_begin = 0; g_layer_end = 1 << 30; }
+};
 
 struct ProfRec { cudaEvent_t a, b; int id; };
 static thread_local bool g_prof_on = false;
@@ -534,6 +540,7 @@ scd_status_t scd_encode(const scd_plan_t* plan, const scd_batch_t* batch, const 
     return fail(SCD_E_SHAPE, "kv strides smaller than the tensor");
   if (!plan->patches.empty() && src->h_token_stride < m.d_model) return fail(SCD_E_SHAPE, "h_token_stride < d_model");
   for (const SegPlan& sp : plan->segs) {
+    if (!layer_in_window(sp.layer)) continue;
     const void* a = sp.branch == SCD_BRANCH_K ? src->k[sp.layer] : sp.branch == SCD_BRANCH_V ? src->v[sp.layer] : src->h[sp.layer];
     if (!a) return fail(SCD_E_ARG, "source state of layer %d branch %d is NULL", sp.layer, sp.branch);
     if (!aligned(a, 16)) return fail(SCD_E_ALIGN, "source state of layer %d not 16-byte aligned", sp.layer);
@@ -546,6 +553,7 @@ scd_status_t scd_encode(const scd_plan_t* plan, const scd_batch_t* batch, const 
   BatchDev bd = batch_dev(plan, batch, false);
   RopeDev rd = rope_dev(plan, true);
   for (const SegPlan& sp : plan->segs) {
+    if (!layer_in_window(sp.layer)) continue;
     GemmSeg g{};
     const int key = sp.layer * 3 + sp.branch;
     if (sp.branch == SCD_BRANCH_H) {
@@ -574,7 +582,7 @@ static scd_status_t check_pools(const scd_plan_t* plan, const scd_paged_kv_t* kv
   if (!kv || !kv->k_pool || !kv->v_pool) return fail(SCD_E_ARG, "kv pools are NULL");
   if (kv->n_blocks < 1) return fail(SCD_E_ARG, "n_blocks must be positive");
   for (int l = 0; l < plan->model.n_layers; ++l) {
-    if (plan->kind[l] != want_kind) continue;
+    if (plan->kind[l] != want_kind || !layer_in_window(l)) continue;
     if (!kv->k_pool[l] || !kv->v_pool[l]) return fail(SCD_E_ARG, "pool of layer %d is NULL", l);
     if (!aligned(kv->k_pool[l], 16) || !aligned(kv->v_pool[l], 16))
       return fail(SCD_E_ALIGN, "pool of layer %d not 16-byte aligned", l);
@@ -602,7 +610,7 @@ scd_status_t scd_reuse_decode(const scd_plan_t* plan, const scd_batch_t* batch, 
   BatchDev bd = batch_dev(plan, batch, true);
   RopeDev rd = rope_dev(plan, false);
   for (const SegPlan& sp : plan->segs) {
-    if (sp.branch == SCD_BRANCH_H) continue;
+    if (sp.branch == SCD_BRANCH_H || !layer_in_window(sp.layer)) continue;
     const int key = sp.layer * 3 + sp.branch;
     GemmSeg g{};
     g.a = (const char*)codes + lay.off[key]; g.lda = sp.rank;
@@ -661,6 +669,7 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
   RopeDev rd = rope_dev(plan, false);
   const bool rms = m.patch_norm == SCD_NORM_RMS;
   for (const PatchPlan& pp : plan->patches) {
+    if (!layer_in_window(pp.layer)) continue;
     const int key = pp.layer * 3 + SCD_BRANCH_H;
     GemmSeg g1{};
     g1.a = (const char*)codes + lay.off[key]; g1.lda = pp.r_h;
@@ -681,6 +690,39 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
     SCD_CUDA(simt_gemm(g3, EPI_KV, A_PLAIN, m.state_dtype, m.code_dtype, bd, rd, (cudaStream_t)stream));
   }
   return SCD_OK;
+}
+
+// ---------------------------------------------------------------------------------
+// layer-streamed variants: the same calls restricted to layers [layer_begin, layer_end), so
+// that encode of later layers, transport of a layer's code segments (scd_plan_code_segment) and decode of earlier
+// layers can overlap on different streams -- Eq. 3's three terms pipelined.  Segments and pools of
+// layers outside the window are neither read, written nor validated.
+// ---------------------------------------------------------------------------------
+static scd_status_t check_window(const scd_plan_t* plan, int32_t b, int32_t e) {
+  if (!plan) return fail(SCD_E_ARG, "plan is NULL");
+  if (b < 0 || e < b || e > plan->model.n_layers) return fail(SCD_E_ARG, "layer window [%d, %d) outside [0, %d]", b, e, plan->model.n_layers);
+  return SCD_OK;
+}
+scd_status_t scd_encode_layers(const scd_plan_t* plan, const scd_batch_t* batch, const scd_src_t* src, void* codes,
+                               int32_t layer_begin, int32_t layer_end, void* stream) {
+  scd_status_t st = check_window(plan, layer_begin, layer_end);
+  if (st != SCD_OK) return st;
+  LayerWindow w(layer_begin, layer_end);
+  return scd_encode(plan, batch, src, codes, stream);
+}
+scd_status_t scd_reuse_decode_layers(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
+                                     const scd_paged_kv_t* kv, int32_t layer_begin, int32_t layer_end, void* stream) {
+  scd_status_t st = check_window(plan, layer_begin, layer_end);
+  if (st != SCD_OK) return st;
+  LayerWindow w(layer_begin, layer_end);
+  return scd_reuse_decode(plan, batch, codes, kv, stream);
+}
+scd_status_t scd_patch_layers(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes, const scd_paged_kv_t* kv,
+                              void* workspace, size_t workspace_bytes, int32_t layer_begin, int32_t layer_end, void* stream) {
+  scd_status_t st = check_window(plan, layer_begin, layer_end);
+  if (st != SCD_OK) return st;
+  LayerWindow w(layer_begin, layer_end);
+  return scd_patch(plan, batch, codes, kv, workspace, workspace_bytes, stream);
 }
 
 }  // extern "C"

@@ -131,6 +131,8 @@ namespace scd {
 // ---- error plumbing (scd_host.cu) -------------------------------------------------
 scd_status_t fail(scd_status_t st, const char* fmt, ...);
 void count_launch();
+// layer window of the running hot call: the *_layers entry points restrict a call to [layer_begin, layer_end)
+bool layer_in_window(int layer);
 // profiling hooks (scd_profile_enable): bracket one launch with events on `s`
 void prof_begin(cudaStream_t s);
 void prof_end(cudaStream_t s, int kernel_id);

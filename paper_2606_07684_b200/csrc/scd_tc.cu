@@ -1012,10 +1012,11 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
   size_t i = 0;
   const size_t nseg = p->segs.size();
   while (i < nseg) {
-    // a launch = run of segments with the same branch, rank and width
+    if (!layer_in_window(p->segs[i].layer)) { ++i; continue; }
+    // a launch = run of segments (inside the call's layer window) with the same branch, rank and width
     size_t j = i;
     while (j < nseg && j - i < (size_t)TC_MAX_SEGS && p->segs[j].branch == p->segs[i].branch &&
-           p->segs[j].rank == p->segs[i].rank)
+           p->segs[j].rank == p->segs[i].rank && layer_in_window(p->segs[j].layer))
       ++j;
     const SegPlan& s0 = p->segs[i];
     static thread_local TcParams P;
@@ -1077,7 +1078,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
   size_t i = 0;
   std::vector<int> reuse;
   for (int q = 0; q < nseg_all; ++q)
-    if (p->segs[q].branch != SCD_BRANCH_H) reuse.push_back(q);
+    if (p->segs[q].branch != SCD_BRANCH_H && layer_in_window(p->segs[q].layer)) reuse.push_back(q);
   while (i < reuse.size()) {
     size_t j = i;
     while (j < reuse.size() && j - i < (size_t)TC_MAX_SEGS && p->segs[reuse[j]].rank == p->segs[reuse[i]].rank) ++j;
@@ -1156,9 +1157,10 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
   if (group > TC_MAX_SEGS) group = TC_MAX_SEGS;
   size_t j0 = 0;
   while (j0 < p->patches.size()) {
+    if (!layer_in_window(p->patches[j0].layer)) { ++j0; continue; }
     size_t j1 = j0;
     while (j1 < p->patches.size() && j1 - j0 < (size_t)group && p->patches[j1].r_h == p->patches[j0].r_h &&
-           p->patches[j1].d_a == p->patches[j0].d_a)
+           p->patches[j1].d_a == p->patches[j0].d_a && layer_in_window(p->patches[j1].layer))
       ++j1;
     const PatchPlan& p0 = p->patches[j0];
     const int g = (int)(j1 - j0);

@@ -78,16 +78,17 @@ class CodecProblem:
         return k, v, h
 
     # ---- the three hot calls ---------------------------------------------------------
-    def encode(self, k, v, h, stream=None) -> int:
+    def encode(self, k, v, h, stream=None, layers=None) -> int:
         cfg = self.cfg
-        return B.scd_encode(self.plan, self.bdesc, k, v, h, self.codes, cfg.D, cfg.head_dim, cfg.d_model, stream)
+        return B.scd_encode(self.plan, self.bdesc, k, v, h, self.codes, cfg.D, cfg.head_dim, cfg.d_model, stream, layers)
 
-    def reuse_decode(self, stream=None) -> int:
-        return B.scd_reuse_decode(self.plan, self.bdesc, self.codes, self.k_pool, self.v_pool, self.batch.n_blocks, stream)
+    def reuse_decode(self, stream=None, layers=None) -> int:
+        return B.scd_reuse_decode(self.plan, self.bdesc, self.codes, self.k_pool, self.v_pool, self.batch.n_blocks, stream,
+                                  layers)
 
-    def patch(self, stream=None) -> int:
+    def patch(self, stream=None, layers=None) -> int:
         return B.scd_patch(self.plan, self.bdesc, self.codes, self.k_pool, self.v_pool, self.batch.n_blocks,
-                           self.workspace, stream)
+                           self.workspace, stream, layers)
 
     # ---- views ---------------------------------------------------------------------
     def code_view(self, layer: int, branch: int):

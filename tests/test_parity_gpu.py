@@ -210,6 +210,43 @@ def test_patch_with_a_one_layer_workspace(cuda_device):
     P.check_patch(prob)
 
 
+@pytest.mark.parametrize("name", ["tiny", "llama3_8b_8k", "mistral_7b_32k_fp8"])
+def test_layer_streamed_calls_give_the_same_bits(name, cuda_device):
+    """scd_*_layers: the path run window by window -- [0,1), [1,3), [3,L), with the source pointers
+    of the other layers withheld -- writes exactly the code and pool bits of the three whole calls; an empty window and a
+    window without REUSE / PATCH layers are no-ops; a bad window is SCD_E_ARG."""
+    from paper_2606_07684_b200 import binding as B
+    cfg = MINI[name] if name == "tiny" else MINI[name].scaled(n_layers=5, patch_layers=(1, 4), seqlens=(300, 45))
+    L = cfg.n_layers
+    prob = _problem(cfg, cuda_device)
+    k, v, h = prob.make_sources()
+    if prob.model.k_is_roped:
+        k = P.roped_producer_k(prob, k)
+    prob.alloc_pools()
+    prob.encode(k, v, h); prob.reuse_decode(); prob.patch()
+    torch.cuda.synchronize()
+    codes_full = prob.codes.clone()
+    pools_full = [t.clone() for t in prob.k_pool + prob.v_pool]
+    prob.codes.zero_()
+    prob.alloc_pools()
+    only = lambda ts, b, e: [t if b <= i < e else None for i, t in enumerate(ts)]
+    windows = [(0, 1), (1, 3), (3, L)] if L > 3 else [(0, 1), (1, L)]
+    for b, e in windows:                                 # producer side, group by group
+        prob.encode(only(k, b, e), only(v, b, e), only(h, b, e), layers=(b, e))
+    for b, e in reversed(windows):                       # consumer side, any order
+        prob.reuse_decode(layers=(b, e))
+        prob.patch(layers=(b, e))
+    assert prob.encode(k, v, h, layers=(2, 2)) == 0      # empty window: nothing launched
+    torch.cuda.synchronize()
+    assert torch.equal(prob.codes, codes_full)
+    for want, got in zip(pools_full, prob.k_pool + prob.v_pool):
+        bits = torch.int32 if want.dtype == torch.float32 else torch.int16
+        assert torch.equal(want.view(bits), got.view(bits))
+    with pytest.raises(B.ScdError) as err:
+        prob.reuse_decode(layers=(3, L + 1))
+    assert err.value.status == 1
+
+
 @pytest.mark.parametrize("state", ["f32", "bf16"])
 def test_edge_batches(state, cuda_device):
     """Ragged lengths that are not multiples of 16 / 128, a 1-token request, position offsets,
