@@ -259,6 +259,67 @@ def run_ours(args, cfg):
     for kid, ms in recs:
         by_kernel.setdefault(kid, []).append(ms)
 
+    # ---- optional: layer-streamed pipeline (scd_*_layers) ----
+    # Producer encodes a group of layers, the group's code segments cross a stand-in link (device-to-device copy into
+    # the consumer's code buffer), the consumer decodes / patches the group -- on three streams, against the same four
+    # steps run whole and back to back.  One GPU plays both sides, so only the copy can truly overlap.
+    streamed = None
+    if args.stream_layers > 0:
+        G, L = args.stream_layers, cfg.n_layers
+        segs = {l: [prob.plan.code_segment(l, br, T) for br in ((2,) if l in cfg.patch_layers else (0, 1))] for l in range(L)}
+        cb = {0: 4, 1: 2, 2: 1}[cfg.code_dtype]
+        rx_codes = torch.zeros_like(prob.codes)
+
+        def link(l0, l1):
+            for l in range(l0, l1):
+                for off, soff, r in segs[l]:
+                    n = T * r * cb
+                    rx_codes[off:off + n].copy_(prob.codes[off:off + n], non_blocking=True)
+                    if cfg.code_dtype == 2:
+                        rx_codes[soff:soff + 4 * T].copy_(prob.codes[soff:soff + 4 * T], non_blocking=True)
+
+        s_link, s_rx = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
+        tx_codes = prob.codes
+
+        def whole():
+            prob.codes = tx_codes
+            prob.encode(k, v, h)
+            link(0, L)
+            prob.codes = rx_codes
+            prob.reuse_decode(); prob.patch()
+            prob.codes = tx_codes
+
+        def pipelined():
+            for l0 in range(0, L, G):
+                l1 = min(L, l0 + G)
+                prob.codes = tx_codes
+                prob.encode(k, v, h, layers=(l0, l1))
+                e1 = ev(); e1.record(stream)
+                s_link.wait_event(e1)
+                with torch.cuda.stream(s_link):
+                    link(l0, l1)
+                    e2 = ev(); e2.record(s_link)
+                s_rx.wait_event(e2)
+                prob.codes = rx_codes
+                prob.reuse_decode(stream=s_rx, layers=(l0, l1))
+                prob.patch(stream=s_rx, layers=(l0, l1))
+            prob.codes = tx_codes
+            e3 = ev(); e3.record(s_rx)
+            stream.wait_event(e3)
+
+        res = {}
+        for name_, fn_ in (("whole_calls_ms", whole), ("pipelined_ms", pipelined)):
+            fn_(); fn_()
+            torch.cuda.synchronize()
+            a, b = ev(), ev()
+            a.record(stream)
+            for _ in range(5):
+                fn_()
+            b.record(stream)
+            torch.cuda.synchronize()
+            res[name_] = a.elapsed_time(b) / 5
+        streamed = {"layers_per_group": G, **res, "link": "device-to-device copy of the group's code segments"}
+
     # ---- e2e: host buffers in, host buffers out ----
     e2e = None
     if not args.no_e2e:
@@ -400,7 +461,7 @@ def run_ours(args, cfg):
         "kv_tokens_per_s_reuse_plus_patch": tokens / ((dec_ms + pat_ms) * 1e-3),
         "kv_gbs_written": costs["kv_bytes_written"] * world / ((dec_ms + pat_ms) * 1e-3) / 1e9,
         "reuse_decode_tokens_per_s": tokens / (dec_ms * 1e-3) if dec_ms else None,
-        "gpu_launches": launches, "wall_s_timed_region": t_wall,
+        "gpu_launches": launches, "wall_s_timed_region": t_wall, "layer_streamed": streamed,
         "clocks": clocks, "roofline": roofline, "rooflines": rooflines,
     }
     if e2e:
@@ -427,6 +488,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--rank", type=int, default=0, help="override the config's rank (config 5 rank sweep)")
+    ap.add_argument("--stream-layers", type=int, default=0,
+                    help="also time the layer-streamed pipeline (scd_*_layers) with this many layers per group")
     ap.add_argument("--per-head-rank", type=int, default=0,
                     help="REUSE layers in the paper's per-head reading (one d_h x r map per layer, PAPER.md:102) with this r")
     args = ap.parse_args()
