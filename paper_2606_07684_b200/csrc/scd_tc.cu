@@ -47,12 +47,12 @@ struct __align__(8) TcBarriers {
 // the bias straight from L1/L2 instead of a per-warp shared copy: that is the room for a fourth stage.
 static int tc_sub_n(int epi, bool compact) { return (epi == EPI_U || compact) ? 64 : SUB_N; }
 static int tc_vec_warp_bytes(int epi, bool compact) { return (epi == EPI_U || epi == EPI_CODES || compact) ? 0 : VEC_WARP_BYTES; }
-static int tc_stg_warp_bytes(int epi, int block_n, bool compact) {
+static int tc_stg_warp_bytes(int epi, int block_n, bool compact, int out_eb) {
   if (compact) return 32 * 128;
   if (epi == EPI_KV) return STG_WARP_BYTES;
   const int cols = (block_n % 64) == 0 ? block_n / 2 : block_n;      // the warp pair splits the columns (gran = 32)
   const int sub = cols < tc_sub_n(epi, false) ? cols : tc_sub_n(epi, false);
-  return 32 * ((sub * 2 + 127) & ~127);
+  return 32 * ((sub * out_eb + 127) & ~127);       // out_eb: 1 for e4m3 codes, else 2
 }
 static size_t tc_smem_bytes(int block_n, int stages, int stg_warp_bytes, int vec_warp_bytes) {
   return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) +
@@ -941,7 +941,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
                        (P.N % 256) == 0;
   P.kv_compact = compact ? 1 : 0;
   P.sub_n = tc_sub_n(EPI, compact);
-  P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n, compact);
+  P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n, compact, (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2);
   P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
   P.a_prefetch = (EPI == EPI_CODES) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
