@@ -114,7 +114,9 @@ typedef struct {
 typedef struct {
   int32_t n_seqs, total_tokens, max_seqlen, max_pages_per_seq;
   const int32_t *cu_seqlens;         /* [n_seqs + 1]                                     */
-  const int32_t *page_table;         /* [n_seqs, max_pages_per_seq] block ids, unused -1 */
+  const int32_t *page_table;         /* [n_seqs, max_pages_per_seq] block ids, unused -1; the table lives on the
+                                        device and is not validated by the host: a token whose page id is outside
+                                        [0, n_blocks) is skipped (its row is not written), never stored out of the pool */
   const int32_t *pos_offset;         /* [n_seqs] first position id, or NULL (= 0)        */
   int32_t max_pos_offset;            /* HOST upper bound on pos_offset[] (0 if NULL)     */
 } scd_batch_t;

@@ -65,7 +65,10 @@ __device__ __forceinline__ void row_to_pos_slot(const BatchDev& batch, int row, 
   slot = -1;
   if (batch.page_table) {
     int page = __ldg(batch.page_table + (size_t)lo * batch.max_pages_per_seq + t / batch.block_size);
-    slot = (long long)page * batch.block_size + t % batch.block_size;
+    // page tables live on the device, so the host cannot validate them: a page id outside the pool (the -1 of an
+    // unused entry reached through an inconsistent cu_seqlens, or a stale id) leaves slot = -1 and the row unwritten
+    if (page >= 0 && (batch.n_blocks <= 0 || page < batch.n_blocks))
+      slot = (long long)page * batch.block_size + t % batch.block_size;
   }
 }
 

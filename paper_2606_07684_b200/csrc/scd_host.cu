@@ -192,7 +192,7 @@ static scd_status_t check_batch(const scd_plan_t* p, const scd_batch_t* b, bool 
   return SCD_OK;
 }
 
-static BatchDev batch_dev(const scd_plan_t* p, const scd_batch_t* b, bool pages) {
+static BatchDev batch_dev(const scd_plan_t* p, const scd_batch_t* b, bool pages, int n_blocks = 0) {
   BatchDev d;
   d.cu_seqlens = b->cu_seqlens;
   d.page_table = pages ? b->page_table : nullptr;
@@ -201,6 +201,7 @@ static BatchDev batch_dev(const scd_plan_t* p, const scd_batch_t* b, bool pages)
   d.total_tokens = b->total_tokens;
   d.max_pages_per_seq = b->max_pages_per_seq;
   d.block_size = p->model.block_size;
+  d.n_blocks = n_blocks;
   return d;
 }
 
@@ -221,14 +222,17 @@ static bool aligned(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
 // fp32 epilogue vectors are read with 16-byte loads up to one tile (256 columns) past N
 static const size_t kVecPad = 256 * sizeof(float);
 
+// zero-filled on the plan's stream: the repack kernels that write the same buffers are enqueued on that stream too, so
+// the fill is ordered before them even when it is a non-blocking stream (a legacy-stream cudaMemset would not be)
 template <typename T>
-static scd_status_t dev_alloc(scd_plan_t* p, T** out, size_t bytes) {
+static scd_status_t dev_alloc(scd_plan_t* p, T** out, size_t bytes, cudaStream_t s) {
   void* ptr = nullptr;
   cudaError_t e = cudaMalloc(&ptr, bytes ? bytes : 16);
   if (e != cudaSuccess) return fail(e == cudaErrorMemoryAllocation ? SCD_E_NOMEM : SCD_E_CUDA, "cudaMalloc(%zu): %s",
                                     bytes, cudaGetErrorString(e));
   p->allocs.push_back(ptr);
-  cudaMemset(ptr, 0, bytes ? bytes : 16);
+  e = cudaMemsetAsync(ptr, 0, bytes ? bytes : 16, s);
+  if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaMemsetAsync(%zu): %s", bytes, cudaGetErrorString(e));
   *out = (T*)ptr;
   return SCD_OK;
 }
@@ -242,12 +246,12 @@ static scd_status_t build_plan(scd_plan_t* p, const scd_layer_desc_t* layers, cu
 
   // RoPE tables (fp64 angles -> fp32 cos/sin)
   const size_t tbytes = (size_t)m.max_position * (m.head_dim / 2) * sizeof(float2);
-  if ((st = dev_alloc(p, &p->rope_cons, tbytes)) != SCD_OK) return st;
+  if ((st = dev_alloc(p, &p->rope_cons, tbytes, s)) != SCD_OK) return st;
   SCD_CUDA(prep_rope_table(p->rope_cons, m.max_position, m.head_dim, m.rope_theta_consumer, s));
   if (m.rope_theta_producer == m.rope_theta_consumer) {
     p->rope_prod = p->rope_cons;
   } else {
-    if ((st = dev_alloc(p, &p->rope_prod, tbytes)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &p->rope_prod, tbytes, s)) != SCD_OK) return st;
     SCD_CUDA(prep_rope_table(p->rope_prod, m.max_position, m.head_dim, m.rope_theta_producer, s));
   }
 
@@ -268,18 +272,18 @@ static scd_status_t build_plan(scd_plan_t* p, const scd_layer_desc_t* layers, cu
       if (br != SCD_BRANCH_H && !dec) return fail(SCD_E_ARG, "layer %d branch %d: decoder is NULL", l, br);
       SegPlan sp{};
       sp.layer = l; sp.branch = br; sp.rank = r; sp.width = width; sp.seg_index = (int)p->segs.size();
-      if ((st = dev_alloc(p, &sp.enc_t, (size_t)r * width * es)) != SCD_OK) return st;
+      if ((st = dev_alloc(p, &sp.enc_t, (size_t)r * width * es, s)) != SCD_OK) return st;
       SCD_CUDA(prep_transpose(enc, sp.enc_t, width, r, sd, s));            // [width, r] -> [r, width]
-      if ((st = dev_alloc(p, &sp.enc_c, (size_t)r * 4 + kVecPad)) != SCD_OK) return st;
+      if ((st = dev_alloc(p, &sp.enc_c, (size_t)r * 4 + kVecPad, s)) != SCD_OK) return st;
       SCD_CUDA(prep_mean_proj(mu_s, enc, sp.enc_c, width, r, sd, s));
       if (mu_s) {
-        if ((st = dev_alloc(p, &sp.mean_src, (size_t)width * 4)) != SCD_OK) return st;
+        if ((st = dev_alloc(p, &sp.mean_src, (size_t)width * 4, s)) != SCD_OK) return st;
         SCD_CUDA(prep_copy_f32(mu_s, sp.mean_src, width, s));
       }
       if (dec) {
-        if ((st = dev_alloc(p, &sp.dec_t, (size_t)D * r * es)) != SCD_OK) return st;
+        if ((st = dev_alloc(p, &sp.dec_t, (size_t)D * r * es, s)) != SCD_OK) return st;
         SCD_CUDA(prep_transpose(dec, sp.dec_t, r, D, sd, s));              // [r, D] -> [D, r]
-        if ((st = dev_alloc(p, &sp.mean_dst, (size_t)D * 4 + kVecPad)) != SCD_OK) return st;
+        if ((st = dev_alloc(p, &sp.mean_dst, (size_t)D * 4 + kVecPad, s)) != SCD_OK) return st;
         SCD_CUDA(prep_copy_f32(mu_d, sp.mean_dst, D, s));
       }
       p->seg_of[(size_t)l * 3 + br] = sp.seg_index;
@@ -295,19 +299,19 @@ static scd_status_t build_plan(scd_plan_t* p, const scd_layer_desc_t* layers, cu
     if (m.patch_norm == SCD_NORM_RMS && !L.norm_gamma) return fail(SCD_E_ARG, "layer %d: norm_gamma is NULL", l);
     PatchPlan pp{};
     pp.layer = l; pp.r_h = L.r_h; pp.d_a = L.d_aligner; pp.h_seg = p->seg_of[(size_t)l * 3 + SCD_BRANCH_H];
-    if ((st = dev_alloc(p, &pp.w1_t, (size_t)pp.d_a * pp.r_h * es)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.w1_t, (size_t)pp.d_a * pp.r_h * es, s)) != SCD_OK) return st;
     SCD_CUDA(prep_transpose(L.w1, pp.w1_t, pp.r_h, pp.d_a, sd, s));        // [r_h, d_a] -> [d_a, r_h]
-    if ((st = dev_alloc(p, &pp.b1, (size_t)pp.d_a * 4 + kVecPad)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.b1, (size_t)pp.d_a * 4 + kVecPad, s)) != SCD_OK) return st;
     SCD_CUDA(prep_to_f32(L.b1, pp.b1, pp.d_a, sd, s));
-    if ((st = dev_alloc(p, &pp.w2_t, (size_t)d * pp.d_a * es)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.w2_t, (size_t)d * pp.d_a * es, s)) != SCD_OK) return st;
     SCD_CUDA(prep_transpose(L.w2, pp.w2_t, pp.d_a, d, sd, s));             // [d_a, d] -> [d, d_a]
-    if ((st = dev_alloc(p, &pp.b2, (size_t)d * 4 + kVecPad)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.b2, (size_t)d * 4 + kVecPad, s)) != SCD_OK) return st;
     SCD_CUDA(prep_to_f32(L.b2, pp.b2, d, sd, s));
-    if ((st = dev_alloc(p, &pp.wkv, (size_t)2 * D * d * es)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.wkv, (size_t)2 * D * d * es, s)) != SCD_OK) return st;
     const void* gamma = m.patch_norm == SCD_NORM_RMS ? L.norm_gamma : nullptr;
     SCD_CUDA(prep_fold_gamma(L.w_k, gamma, pp.wkv, D, d, sd, s));
     SCD_CUDA(prep_fold_gamma(L.w_v, gamma, (char*)pp.wkv + (size_t)D * d * es, D, d, sd, s));
-    if ((st = dev_alloc(p, &pp.bkv, (size_t)2 * D * 4 + kVecPad)) != SCD_OK) return st;
+    if ((st = dev_alloc(p, &pp.bkv, (size_t)2 * D * 4 + kVecPad, s)) != SCD_OK) return st;
     SCD_CUDA(prep_to_f32(L.b_k, pp.bkv, D, sd, s));
     SCD_CUDA(prep_to_f32(L.b_v, pp.bkv + D, D, sd, s));
     p->patches.push_back(pp);
@@ -461,6 +465,8 @@ scd_status_t scd_plan(const scd_model_desc_t* model, const scd_layer_desc_t* lay
   p->model = *model;
   p->D = model->n_kv_heads * model->head_dim;
   p->sm_count = sms;
+  p->device = dev;
+  if (dev < 0 || dev >= SCD_MAX_DEVICES) { delete p; return fail(SCD_E_UNSUPPORTED, "device ordinal %d >= %d", dev, SCD_MAX_DEVICES); }
   for (int i = 0; i < model->n_layers; ++i) {
     p->kind.push_back(layers[i].kind);
     p->r_k.push_back(layers[i].kind == SCD_REUSE ? layers[i].r_k : 0);
@@ -471,9 +477,7 @@ scd_status_t scd_plan(const scd_model_desc_t* model, const scd_layer_desc_t* lay
     p->head_rank_k.push_back(ph ? user_layers[i].r_k : 0);
     p->head_rank_v.push_back(ph ? user_layers[i].r_v : 0);
   }
-  const char* dbg = getenv("SCD_DEBUG_FORCE_SIMT");
-  p->force_simt = dbg && dbg[0] == '1';
-  p->use_tc = model->state_dtype == SCD_BF16 && !p->force_simt;
+  p->use_tc = model->state_dtype == SCD_BF16;
   if (p->use_tc && (st = tc_supported(p, layers)) != SCD_OK) { scd_plan_destroy(p); return st; }
 
   st = build_plan(p, layers, (cudaStream_t)stream);
@@ -604,10 +608,9 @@ scd_status_t scd_reuse_decode(const scd_plan_t* plan, const scd_batch_t* batch, 
   Layout lay;
   plan_layout(plan, T, &lay);
 
-  // e4m3 codes as the A operand: tensor-core expansion not built yet -> SIMT kernels
   if (plan->use_tc) return tc_reuse_decode(plan, batch, codes, kv, lay.off, lay.soff, (cudaStream_t)stream);
 
-  BatchDev bd = batch_dev(plan, batch, true);
+  BatchDev bd = batch_dev(plan, batch, true, kv->n_blocks);
   RopeDev rd = rope_dev(plan, false);
   for (const SegPlan& sp : plan->segs) {
     if (sp.branch == SCD_BRANCH_H || !layer_in_window(sp.layer)) continue;
@@ -665,7 +668,7 @@ scd_status_t scd_patch(const scd_plan_t* plan, const scd_batch_t* batch, const v
     return tc_patch(plan, batch, codes, kv, ws_act, ws_u, ws_ss, pw.group, pw.act_stride, pw.u_stride, pw.ss_stride, lay.off,
                     lay.soff, (cudaStream_t)stream);
 
-  BatchDev bd = batch_dev(plan, batch, true);
+  BatchDev bd = batch_dev(plan, batch, true, kv->n_blocks);
   RopeDev rd = rope_dev(plan, false);
   const bool rms = m.patch_norm == SCD_NORM_RMS;
   for (const PatchPlan& pp : plan->patches) {

@@ -15,6 +15,8 @@
 
 namespace scd {
 
+constexpr int SCD_MAX_DEVICES = 64;
+
 // ---------------------------------------------------------------------------------
 // Epilogue kinds of the one GEMM shape the whole path reduces to:
 //     C[M, N] = A[M, K] * Bt[N, K]^T      (A, Bt both K-major)
@@ -44,6 +46,7 @@ struct BatchDev {
   const int32_t* page_table;
   const int32_t* pos_offset;   // may be null
   int32_t n_seqs, total_tokens, max_pages_per_seq, block_size;
+  int32_t n_blocks;            // pages in the pool (0 = not checked): a page id outside [0, n_blocks) makes the row's slot -1
 };
 
 // RoPE geometry.  Tables hold (cos, sin) of p * theta^(-2j/d_h), [max_position][d_h/2].
@@ -113,9 +116,8 @@ struct scd_plan {
   float2* rope_prod = nullptr;                        // [max_position][d_h/2]
   float2* rope_cons = nullptr;
   std::vector<void*> allocs;                          // everything cudaMalloc'ed by the plan
-  int32_t D = 0, sm_count = 0;
+  int32_t D = 0, sm_count = 0, device = 0;            // device: ordinal the plan was created on
   bool use_tc = false;                                // bf16 state -> tcgen05 kernels
-  bool force_simt = false;                            // SCD_DEBUG_FORCE_SIMT=1 (debug only)
   // tcgen05 path: plan-owned TMA descriptors of the B operands in device memory
   // ([0,nseg) encoders, [nseg,2nseg) decoders, then 3 per PATCH layer)
   void* tc_bmaps = nullptr;

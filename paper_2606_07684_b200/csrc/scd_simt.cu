@@ -174,7 +174,7 @@ simt_gemm_kernel(GemmSeg g, int a_mode, int code_dtype, BatchDev batch, RopeDev 
           }
           TS* pool = (TS*)(col < g.split ? g.out0 : g.out1);
           int pc = col < g.split ? col : col - g.split;
-          pool[(size_t)s_slot[r] * g.pool_width + pc] = from_float<TS>(v);
+          if (s_slot[r] >= 0) pool[(size_t)s_slot[r] * g.pool_width + pc] = from_float<TS>(v);   // -1: page id outside the pool
         }
       }
     }

@@ -438,8 +438,9 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           long long slot;
           row_to_pos_slot(P.batch, row, ri.pos, slot);
           const bool to1 = n0 >= P.split;
-          ri.row_ptr = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
-                       ((unsigned long long)slot * P.pool_width + (to1 ? n0 - P.split : n0)) * 2ull;
+          if (slot >= 0)                                  // -1: page id outside the pool -> the row is not written
+            ri.row_ptr = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
+                         ((unsigned long long)slot * P.pool_width + (to1 ? n0 - P.split : n0)) * 2ull;
         } else {
           ri.row_ptr = (unsigned long long)sg.out0 + ((unsigned long long)row * P.N + n0) * (unsigned long long)out_eb;
         }
@@ -870,8 +871,11 @@ static int pick_block_n_div(int n) {            // largest tile width that divid
     if (n % b == 0) return b;
   return 0;
 }
-static int pick_block_n_cover(int n) {          // smallest multiple of 16 covering n, capped at 256
-  int b = (n + 15) / 16 * 16;
+// Smallest multiple of 32 covering n, capped at 256.  32, not the MMA's own granularity of 16: the epilogue reads TMEM
+// in 32-column chunks, and TMEM is not cleared between kernels -- every column it reads must have been written by this
+// tile's MMA (columns in [N, block_n) are written as exact zeros: their B rows are zero-filled by the TMA).
+static int pick_block_n_cover(int n) {
+  int b = (n + 31) / 32 * 32;
   return b > 256 ? 256 : b;
 }
 
@@ -913,16 +917,15 @@ scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
   void* d = nullptr;
   if (cudaMalloc(&d, maps.size() * sizeof(CUtensorMap) + 64) != cudaSuccess) return fail(SCD_E_NOMEM, "cudaMalloc(tensor maps)");
   p->allocs.push_back(d);
-  if (cudaMemcpy(d, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess)
-    return fail(SCD_E_CUDA, "cudaMemcpy(tensor maps)");
+  // stream-ordered on the plan's stream (pageable source: staged before the call returns), like every other plan write
+  if (cudaMemcpyAsync(d, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice, s) != cudaSuccess)
+    return fail(SCD_E_CUDA, "cudaMemcpyAsync(tensor maps)");
   p->tc_bmaps = d;
   void* sc = nullptr;
   if (cudaMalloc(&sc, KV_SCHED_SETS * 2 * sizeof(int32_t)) != cudaSuccess) return fail(SCD_E_NOMEM, "cudaMalloc(kv scheduler)");
   p->allocs.push_back(sc);
-  if (cudaMemset(sc, 0, KV_SCHED_SETS * 2 * sizeof(int32_t)) != cudaSuccess) return fail(SCD_E_CUDA, "cudaMemset(kv scheduler)");
+  if (cudaMemsetAsync(sc, 0, KV_SCHED_SETS * 2 * sizeof(int32_t), s) != cudaSuccess) return fail(SCD_E_CUDA, "cudaMemsetAsync(kv scheduler)");
   p->kv_sched = (int32_t*)sc;
-
-  (void)s;
   return SCD_OK;
 }
 
@@ -952,11 +955,12 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
     if (msb < P.m_tiles) P.msb = msb;
   }
   const size_t smem = tc_smem_bytes(P.block_n, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
-  static thread_local size_t configured = 0;   // per instantiation
-  if (configured < smem) {
+  // the attribute belongs to (function, device): cached per instantiation and device ordinal
+  static std::atomic<size_t> configured[SCD_MAX_DEVICES];
+  if (configured[p->device].load(std::memory_order_relaxed) < smem) {
     cudaError_t e = cudaFuncSetAttribute(tc_gemm_kernel<EPI, AMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(smem %zu): %s", smem, cudaGetErrorString(e));
-    configured = smem;
+    configured[p->device].store(smem, std::memory_order_relaxed);
   }
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
@@ -968,7 +972,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   return SCD_OK;
 }
 
-static void fill_common(const scd_plan_t* p, const scd_batch_t* b, bool pages, bool producer, TcParams& P) {
+static void fill_common(const scd_plan_t* p, const scd_batch_t* b, bool pages, bool producer, TcParams& P, int n_blocks = 0) {
   memset(&P, 0, sizeof(P));
   P.b_maps = (const CUtensorMap*)p->tc_bmaps;
   P.batch.cu_seqlens = b->cu_seqlens;
@@ -978,6 +982,7 @@ static void fill_common(const scd_plan_t* p, const scd_batch_t* b, bool pages, b
   P.batch.total_tokens = b->total_tokens;
   P.batch.max_pages_per_seq = b->max_pages_per_seq;
   P.batch.block_size = p->model.block_size;
+  P.batch.n_blocks = n_blocks;
   {
     // frequencies as Q0.32 fractions of a turn, from fp64 (exact modular angle arithmetic in the kernel)
     const double theta = producer ? p->model.rope_theta_producer : p->model.rope_theta_consumer;
@@ -1084,7 +1089,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
     while (j < reuse.size() && j - i < (size_t)TC_MAX_SEGS && p->segs[reuse[j]].rank == p->segs[reuse[i]].rank) ++j;
     const SegPlan& s0 = p->segs[reuse[i]];
     static thread_local TcParams P;
-    fill_common(p, batch, true, false, P);
+    fill_common(p, batch, true, false, P, kv->n_blocks);
     P.n_segs = (int)(j - i);
     P.N = p->D;
     P.K = s0.rank;
@@ -1129,7 +1134,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
     P.prof_id = SCD_PROF_REUSE_DECODE;
     P.head_rank = m.reuse_per_head ? s0.rank / m.n_kv_heads : 0;
     if (e4) st = launch_tc<EPI_KV, A_CODES>(p, P, s);       // operand expansion in shared memory (generic kernel)
-    else st = tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
+    else st = tc_kv_eligible(p, P) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
     if (st != SCD_OK) return st;
     i = j;
   }
@@ -1197,7 +1202,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     P.prof_id = SCD_PROF_PATCH_GEMM2;
     if ((st = launch_tc<EPI_U, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     // GEMM-3: [T, d] x [d, 2D] per layer
-    fill_common(p, batch, true, false, P);
+    fill_common(p, batch, true, false, P, kv->n_blocks);
     P.n_segs = g; P.N = 2 * D; P.K = d; P.block_n = pick_block_n_div(D);
     P.split = D; P.pool_width = D; P.n_partials = n_partials; P.rms_dim = d; P.rms_eps = m.rms_eps;
     for (int q = 0; q < g; ++q) {
@@ -1214,7 +1219,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     // long K (d_model >= 1024): the generic kernel with the compact epilogue runs four pipeline stages where the
     // paged-KV kernel has room for three; short K: the paged-KV kernel's faster epilogue wins
     const bool long_k = G3_GENERIC && d >= 16 * BLOCK_K;
-    if ((st = (!long_k && tc_kv_eligible(p, P, (long long)kv->n_blocks * m.block_size)) ? launch_tc_kv(p, P, s)
+    if ((st = (!long_k && tc_kv_eligible(p, P)) ? launch_tc_kv(p, P, s)
                                                                                        : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK)
       return st;
     j0 = j1;

@@ -113,7 +113,7 @@ __device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterp
 
 // scd_tc_kv.cu: can the specialised paged-KV kernel take this launch?  (head_dim 128, HALF RoPE,
 // 256-column tiles, whole tiles only.)  P.M/N/K/block_n/split/rope fields must be filled.
-bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P, long long pool_slots);
+bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P);
 scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s);
 
 }  // namespace scd

@@ -350,6 +350,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         rs_row = 1.0f;
         if (valid) {
           row_to_pos_slot(P.batch, row, pos, slot);
+          valid = slot >= 0;                                    // -1: page id outside the pool -> the row is not written
           if (sg.rowscale_in) {                                 // NORM_RMS (PATCH GEMM-3; several segments only with DYN)
             float ss = 0.0f;
             for (int p = 0; p < P.n_partials; ++p) ss += __ldg(sg.rowscale_in + (size_t)p * P.M + row);
@@ -477,8 +478,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
 // ---------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------
-bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P, long long pool_slots) {
-  (void)pool_slots;
+bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P) {
   if (p->model.head_dim != 128 || p->model.rope_style != SCD_ROPE_HALF) return false;
   if (P.block_n != KV_BLOCK_N || (P.N % KV_BLOCK_N) || (P.split % KV_BLOCK_N) || P.a_kb_per_head != 0) return false;
   for (int i = 0; i < P.n_segs; ++i) {
@@ -495,12 +495,12 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   if (total <= 0) return SCD_OK;
   P.stages = kv_pick_stages(P.num_kb);
   const size_t smem = kv_smem_bytes(P.stages);
-  static thread_local size_t configured = 0;
-  if (configured < smem) {
+  static std::atomic<size_t> configured[SCD_MAX_DEVICES];      // the attribute belongs to (function, device)
+  if (configured[p->device].load(std::memory_order_relaxed) < smem) {
     cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
-    configured = smem;
+    configured[p->device].store(smem, std::memory_order_relaxed);
   }
   const int grid = std::min(total, p->sm_count);
   // long tiles (K = d_model: PATCH GEMM-3): KV_STATIC_PCT % of an even split is owned statically, the rest is

@@ -11,6 +11,9 @@ from . import binding as B
 from . import workloads as W
 
 
+GUARD_BYTES, GUARD_BYTE = 4096, 0xA5
+
+
 class CodecProblem:
     """One synthetic workload resident on `device`: artifacts, plan, batch, code buffer,
     workspace and sentinel-filled paged pools."""
@@ -19,14 +22,18 @@ class CodecProblem:
                  k_is_roped: bool = True, rope_on_reuse_k: bool = True, patch_norm: int = B.SCD_NORM_RMS,
                  patch_act: int = B.SCD_ACT_SILU, rope_style: int = B.SCD_ROPE_HALF,
                  rope_theta_consumer: Optional[float] = None, use_means: bool = True,
-                 artifacts: Optional[List[W.LayerArtifacts]] = None, per_head_rank: int = 0):
+                 artifacts: Optional[List[W.LayerArtifacts]] = None, per_head_rank: int = 0, gen_device=None):
+        """`gen_device`: where the synthetic tensors are drawn and the bases fitted (default: `device`).  "cpu" keeps
+        the library eigen-solver / QR kernels off the GPU, so that a launch trace of a short run (smoke) shows the
+        codec's own kernels."""
         self.cfg = cfg
         self.device = torch.device(device)
+        self.gen_device = self.device if gen_device is None else torch.device(gen_device)
         self.batch = W.make_batch(cfg, self.device, pos_offset)
         self.T = self.batch.total_tokens
         self.use_means = use_means
         self.arts = artifacts if artifacts is not None else [
-            W.make_layer_artifacts(cfg, l, self.device, total_rows=max(self.T, 1), per_head_rank=per_head_rank)
+            W.make_layer_artifacts(cfg, l, self.gen_device, total_rows=max(self.T, 1), per_head_rank=per_head_rank).to(self.device)
             for l in range(cfg.n_layers)]
         self.per_head_rank = per_head_rank
         max_off = max(pos_offset) if pos_offset is not None else 0
@@ -41,8 +48,12 @@ class CodecProblem:
         self.plan = B.scd_plan(self.model, self.layer_descs)
         torch.cuda.synchronize(self.device)
         self.code_bytes, self.ws_bytes, self.payload_bytes = self.plan.query(self.T)
-        self.codes = torch.zeros(max(self.code_bytes, 128), dtype=torch.uint8, device=self.device)
-        self.workspace = torch.empty(max(self.ws_bytes, 128), dtype=torch.uint8, device=self.device)
+        # both buffers sit in front of GUARD_BYTES of guard and start out filled with GUARD_BYTE, so that tests can see
+        # writes into the padding between code segments, past the last scale segment or past the workspace
+        self._codes_alloc = torch.full((max(self.code_bytes, 128) + GUARD_BYTES,), GUARD_BYTE, dtype=torch.uint8, device=self.device)
+        self.codes = self._codes_alloc[:max(self.code_bytes, 128)]
+        self._ws_alloc = torch.full((max(self.ws_bytes, 128) + GUARD_BYTES,), GUARD_BYTE, dtype=torch.uint8, device=self.device)
+        self.workspace = self._ws_alloc[:max(self.ws_bytes, 128)]
         self.k_pool: List[torch.Tensor] = []
         self.v_pool: List[torch.Tensor] = []
         self.bdesc = B.batch_desc(self.batch.cu_seqlens, self.batch.page_table, self.batch.pos_offset,
@@ -71,10 +82,10 @@ class CodecProblem:
         h: List[Optional[torch.Tensor]] = [None] * L
         for l in range(L):
             if l in cfg.patch_layers:
-                h[l] = W.make_state(cfg, l, 2, self.T, self.device)
+                h[l] = W.make_state(cfg, l, 2, self.T, self.gen_device).to(self.device)
             else:
-                k[l] = W.make_state(cfg, l, 0, self.T, self.device)
-                v[l] = W.make_state(cfg, l, 1, self.T, self.device)
+                k[l] = W.make_state(cfg, l, 0, self.T, self.gen_device).to(self.device)
+                v[l] = W.make_state(cfg, l, 1, self.T, self.gen_device).to(self.device)
         return k, v, h
 
     # ---- the three hot calls ---------------------------------------------------------
@@ -91,6 +102,29 @@ class CodecProblem:
                            self.workspace, stream, layers)
 
     # ---- views ---------------------------------------------------------------------
+    def code_ranges(self):
+        """Byte ranges [begin, end) of the code buffer that scd_encode may write: every segment's codes and scales."""
+        cb = {W.F32: 4, W.BF16: 2, W.E4M3_ROWSCALE: 1}[self.cfg.code_dtype]
+        out = []
+        for l in range(self.cfg.n_layers):
+            for br in ((2,) if self.arts[l].kind == W.PATCH else (0, 1)):
+                off, soff, r = self.plan.code_segment(l, br, self.T)
+                out.append((off, off + self.T * r * cb))
+                if self.cfg.code_dtype == W.E4M3_ROWSCALE:
+                    out.append((soff, soff + self.T * 4))
+        return sorted(out)
+
+    def guard_violations(self):
+        """Bytes outside the writable ranges that no longer hold GUARD_BYTE: (in the code buffer's padding and guard,
+        in the guard after the workspace)."""
+        bad_c, at = 0, 0
+        for b, e in self.code_ranges() + [(self._codes_alloc.numel(), self._codes_alloc.numel())]:
+            if b > at:
+                bad_c += int((self._codes_alloc[at:b] != GUARD_BYTE).sum())
+            at = max(at, e)
+        bad_w = int((self._ws_alloc[self.workspace.numel():] != GUARD_BYTE).sum())
+        return bad_c, bad_w
+
     def code_view(self, layer: int, branch: int):
         """(codes [T, r] tensor view in the code dtype, scales [T] fp32 or None)."""
         off, soff, r = self.plan.code_segment(layer, branch, self.T)

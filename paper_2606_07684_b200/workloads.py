@@ -214,6 +214,11 @@ class LayerArtifacts:
     b_k: Optional[torch.Tensor] = None
     b_v: Optional[torch.Tensor] = None
 
+    def to(self, device) -> "LayerArtifacts":
+        """The same artifacts on another device (e.g. drawn on the CPU, used on the GPU)."""
+        return LayerArtifacts(**{f.name: (v.to(device) if isinstance(v, torch.Tensor) else v)
+                                 for f in dataclasses.fields(self) for v in (getattr(self, f.name),)})
+
 
 def make_layer_artifacts(cfg: WorkloadConfig, layer: int, device, cal_rows: int = 8192,
                          total_rows: Optional[int] = None, per_head_rank: int = 0) -> LayerArtifacts:

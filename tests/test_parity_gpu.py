@@ -51,7 +51,10 @@ def _run_all(prob, rows=None, roped=True):
     P.check_untouched(prob, reuse + patch, slots)
     pat = P.check_patch(prob, rows)
     P.check_reuse_decode(prob, rows)                                       # and PATCH left REUSE layers alone
-    return {"encode": enc["worst_rel_fro"], "reuse": dec["worst_rel_fro"], "patch": pat["worst_rel_fro"]}
+    # nothing outside the code segments / scale segments / workspace was written (padding, tails, guards)
+    assert prob.guard_violations() == (0, 0), f"guard bytes overwritten (code buffer, workspace): {prob.guard_violations()}"
+    used = {k_: round(v_, 3) for d_ in (enc, dec, pat) for k_, v_ in d_.items() if k_ not in ("worst_rel_fro", "slots")}
+    return {"encode": enc["worst_rel_fro"], "reuse": dec["worst_rel_fro"], "patch": pat["worst_rel_fro"], "bounds_used": used}
 
 
 @pytest.mark.parametrize("name", list(MINI))
@@ -149,6 +152,76 @@ def test_ranks_that_are_not_powers_of_two(rank, cuda_device):
     _run_all(_problem(cfg, cuda_device))
 
 
+@pytest.mark.parametrize("rank", [32, 64, 128, 256, 512])
+def test_config5_rank_sweep_mini(rank, cuda_device):
+    """BASELINE.json configs[4] sweeps the per-layer rank over {32, 64, 128, 256, 512}: every one of them on config-5
+    geometry (2 requests, REUSE layers and one PATCH layer).  r = 256 fills the encode's widest tile; r = 512 is the
+    distinct path where a segment's codes span two 256-wide n-tiles of the encode and the decode runs K = 512
+    (8 k-blocks)."""
+    cfg = MINI["llama3_70b_2x16k"].scaled(rank=rank, seqlens=(300, 333), n_layers=3, patch_layers=(1,), d_model=2048)
+    res = _run_all(_problem(cfg, cuda_device))
+    print(rank, res)
+
+
+@pytest.mark.parametrize("rank,d_model", [(16, 1024), (48, 1024), (48, 80), (80, 1024), (112, 528)])
+def test_tile_widths_that_are_not_multiples_of_32_on_dirty_tmem(rank, d_model, cuda_device):
+    """The epilogue reads TMEM 32 columns at a time and TMEM is not cleared between kernels: a tile narrower than the
+    last chunk it reads (e4m3 rank 16 / 48 / 80 / 112 in the row-amax pass; d_model = 80 / 528 in GEMM-2's row sum of
+    squares) must not pick up a previous kernel's accumulators.  A 256-column decode runs first, so every SM's TMEM
+    holds large stale values; a stale value in the amax would show as a wrong e4m3 scale, in the sum of squares as a
+    wrong RMS scale of the PATCH layer."""
+    dirty = _problem(MINI["llama3_8b_8k"].scaled(n_layers=1, patch_layers=(), seqlens=(2048,)), cuda_device)
+    k, v, h = dirty.make_sources()
+    dirty.alloc_pools()
+    dirty.encode(k, v, h)
+    q, _ = dirty.code_view(0, 0)
+    q.mul_(1e4)                                                   # large accumulators left behind in TMEM
+    dirty.reuse_decode()
+    cfg = MINI["mistral_7b_32k_fp8"].scaled(rank=rank, d_model=d_model, n_layers=2, patch_layers=(1,), seqlens=(300,),
+                                            spectrum_k=min(512, d_model))
+    res = _run_all(_problem(cfg, cuda_device))
+    print(rank, d_model, res)
+
+
+def test_plan_built_on_a_non_blocking_stream(cuda_device):
+    """scd_plan enqueues its zero-fills and repacks on the caller's stream; on a non-blocking stream (every
+    torch.cuda.Stream) a legacy-stream memset would be unordered with them and could wipe artifacts.  Busy work on the
+    default stream makes a misordering likely to show."""
+    from paper_2606_07684_b200.harness import CodecProblem
+    cfg = MINI["llama3_8b_8k"].scaled(n_layers=3, patch_layers=(1,), seqlens=(300,), d_model=512)
+    side = torch.cuda.Stream(device=cuda_device)
+    busy = torch.randn(4096, 4096, device=cuda_device)
+    for _ in range(20):
+        busy = busy @ busy * 1e-3                                 # keeps the default (blocking) stream occupied
+    with torch.cuda.stream(side):
+        prob = CodecProblem(cfg, cuda_device)                    # plan on `side` (the binding passes the current stream)
+        res = _run_all(prob)
+    torch.cuda.synchronize()
+    print(res)
+
+
+def test_page_ids_outside_the_pool_are_skipped_not_written(cuda_device):
+    """Page tables live on the device, so the host cannot validate them (include/scd.h): a row whose page id is -1 or
+    >= n_blocks is left unwritten -- never a store outside the pool."""
+    cfg = MINI["llama3_8b_8k"].scaled(n_layers=2, patch_layers=(1,), seqlens=(300, 200), d_model=512)
+    prob = _problem(cfg, cuda_device)
+    k, v, h = prob.make_sources()
+    prob.alloc_pools()
+    prob.encode(k, v, h)
+    torch.cuda.synchronize()
+    slots = O.slot_mapping(P.oracle_batch(prob), cfg.block_size)           # from the intact table
+    prob.batch.page_table[0, 3] = prob.batch.n_blocks + 7                  # rows 48..63 of request 0
+    prob.batch.page_table[1, 0] = -1                                       # rows 0..15 of request 1
+    prob.reuse_decode()
+    prob.patch()
+    torch.cuda.synchronize()
+    bad = np.r_[48:64, 300:316]
+    good = np.setdiff1d(np.arange(prob.T), bad)
+    P.check_untouched(prob, [0, 1], slots[good])                           # the bad rows' slots still hold the sentinel
+    P.check_reuse_decode(prob, good)
+    P.check_patch(prob, good)
+
+
 def test_all_layers_patch_with_mixed_code_ranks(cuda_device):
     """L_patch = all layers (legal), with PATCH layers whose r_h differ: scd_patch runs each GEMM stage for a
     group of consecutive layers of equal (r_h, d_a) as one launch, so ranks 128, 64, 64, 128 exercise groups of 1, 2, 1."""
@@ -227,7 +300,7 @@ def test_layer_streamed_calls_give_the_same_bits(name, cuda_device):
     torch.cuda.synchronize()
     codes_full = prob.codes.clone()
     pools_full = [t.clone() for t in prob.k_pool + prob.v_pool]
-    prob.codes.zero_()
+    prob.codes.fill_(0xA5)                               # the harness' guard pattern (padding bytes are compared too)
     prob.alloc_pools()
     only = lambda ts, b, e: [t if b <= i < e else None for i, t in enumerate(ts)]
     windows = [(0, 1), (1, 3), (3, L)] if L > 3 else [(0, 1), (1, L)]
@@ -323,12 +396,14 @@ FULL_SAMPLE = {"llama3_8b_8k": 384, "llama3_8b_ragged": 256, "mistral_7b_32k_fp8
 
 
 @pytest.mark.slow
-@pytest.mark.parametrize("name", ["llama3_8b_8k", "llama3_8b_ragged", "mistral_7b_32k_fp8", "llama3_70b_2x16k"])
-def test_full_size_sampled_parity(name, cuda_device):
-    """BASELINE.json's full sizes in the launch configuration bench.py times; the oracle
-    recomputes a row sample (first / last rows of every request, ragged tails, seeded random
-    rows -- rows are independent); sentinels checked over the whole pool."""
-    prob = _problem(C[name], cuda_device)
+@pytest.mark.parametrize("name,rank", [("llama3_8b_8k", 0), ("llama3_8b_ragged", 0), ("mistral_7b_32k_fp8", 0),
+                                       ("llama3_70b_2x16k", 0), ("llama3_70b_2x16k", 512)])
+def test_full_size_sampled_parity(name, rank, cuda_device):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (rank 0 = the config's own; 512 = the
+    widest rank of the config-5 sweep); the oracle recomputes a row sample (first / last rows of every request,
+    ragged tails, seeded random rows -- rows are independent); sentinels checked over the whole pool."""
+    cfg = C[name] if not rank else C[name].scaled(rank=rank)
+    prob = _problem(cfg, cuda_device)
     rows = P.sample_rows(prob, FULL_SAMPLE[name])
     res = _run_all(prob, rows=rows, roped=False)
-    print(name, res)
+    print(name, rank, res)
