@@ -69,3 +69,25 @@ def test_rerounded_operand_noise_term_is_a_bound_not_a_blank_cheque():
     assert (real <= extra).all() and real.max() >= 0.1 * extra.min()
     cauchy = 2.0 ** -8 * np.linalg.norm(kt, axis=1)[:, None] * np.linalg.norm(q, axis=0)[None, :]
     assert extra.max() < cauchy.min() / 8.0
+
+
+def test_e4m3_cell_check_accepts_the_oracles_own_codes_and_rejects_a_neighbouring_code():
+    rng = np.random.default_rng(4)
+    z = rng.standard_normal((64, 96)) * (0.97 ** np.arange(96))[None, :]
+    z[5] = 0.0                                                     # all-zero row: scale 1, codes 0
+    q, s = O.pack_codes(z, O.E4M3_ROWSCALE)
+    tiny = np.full(z.shape, 1e-12)
+    assert P.e4m3_cell_check(z, q, s, tiny, "own codes") == 0.0
+    bad = q.copy()
+    bad[10, 3] = bad[10, 3] + 1 if (bad[10, 3] & 0x7F) < 0x7E else bad[10, 3] - 1      # the next code up (or down at the top)
+    with pytest.raises(AssertionError):
+        P.e4m3_cell_check(z, bad, s, tiny, "neighbouring code")
+    flipped = q.copy()
+    flipped[20, 7] ^= 0x80                                         # wrong sign
+    if (q[20, 7] & 0x7F) != 0:
+        with pytest.raises(AssertionError):
+            P.e4m3_cell_check(z, flipped, s, tiny, "wrong sign")
+    # a value just past a rounding boundary may legitimately take either neighbour when the noise allowance covers it
+    z2 = np.array([[448.0, 17.0 + 1e-9]])                          # scale 1; 17 is the midpoint of codes 16 and 18
+    q2 = np.array([[0x7E, O.e4m3_quantize(np.array([16.0]))[0]]], dtype=np.uint8)
+    assert 0.0 < P.e4m3_cell_check(z2, q2, np.ones(1, np.float32), np.full((1, 2), 1e-6), "boundary") <= 1.0
