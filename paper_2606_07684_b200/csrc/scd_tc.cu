@@ -983,6 +983,7 @@ static void fill_common(const scd_plan_t* p, const scd_batch_t* b, bool pages, b
   P.batch.max_pages_per_seq = b->max_pages_per_seq;
   P.batch.block_size = p->model.block_size;
   P.batch.n_blocks = n_blocks;
+  P.pool_slots = (long long)n_blocks * p->model.block_size;
   {
     // frequencies as Q0.32 fractions of a turn, from fp64 (exact modular angle arithmetic in the kernel)
     const double theta = producer ? p->model.rope_theta_producer : p->model.rope_theta_consumer;

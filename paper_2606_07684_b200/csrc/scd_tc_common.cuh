@@ -47,6 +47,7 @@ struct TcParams {
   int32_t head_rank;                  // paged-KV kernel, per-head REUSE: codes per head (A/B are block-diagonal), else 0
   int32_t prof_id;                    // host only: id under which scd_profile_* reports the launch
   int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
+  long long pool_slots;               // paged epilogues: n_blocks * block_size (slot numbers are kept as int32)
 };
 
 constexpr int KV_SCHED_SETS = 64;
@@ -86,6 +87,11 @@ __device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsig
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
   return r;
 }
+__device__ __forceinline__ unsigned long long f2_add(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
 __device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b) {
   unsigned long long r;
   asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
@@ -115,5 +121,6 @@ __device__ __forceinline__ float4 ldg_f4(const float* p) { return __ldg(reinterp
 // 256-column tiles, whole tiles only.)  P.M/N/K/block_n/split/rope fields must be filled.
 bool tc_kv_eligible(const scd_plan_t* p, const TcParams& P);
 scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s);
+
 
 }  // namespace scd

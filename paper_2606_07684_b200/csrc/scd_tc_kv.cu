@@ -30,8 +30,10 @@ namespace {
 constexpr int KV_BLOCK_N = 256;
 constexpr int KV_EPI_WARPS = 16;
 constexpr int KV_B_STAGE_BYTES = KV_BLOCK_N * BLOCK_K * 2;   // 32 KB
-constexpr int KV_STG_BYTES = 4 * 32 * KV_BLOCK_N * 2;        // 4 quadrants x [32 rows x 512 B] = 64 KB
+constexpr int KV_ROW_PITCH = 512;
+constexpr int KV_STG_BYTES = 4 * 32 * KV_ROW_PITCH;          // 4 quadrants x [32 rows x 512 B] = 64 KB
 constexpr int KV_VEC_BYTES = KV_EPI_WARPS * 64 * 4;          // per-warp slice of the tile's mean / bias: 64 floats
+constexpr int KV_SLOT_BYTES = KV_EPI_WARPS * 32 * 4;         // per-warp copy of its quadrant's 32 slot numbers (-1 = no row)
 
 struct __align__(8) KvBarriers {
   uint64_t full[MAX_STAGES], empty[MAX_STAGES];
@@ -43,10 +45,10 @@ struct __align__(8) KvBarriers {
 constexpr int KV_SCHED_SLOTS = 4;
 
 size_t kv_smem_bytes(int stages) {
-  return 1024 + (size_t)stages * (A_STAGE_BYTES + KV_B_STAGE_BYTES) + KV_STG_BYTES + KV_VEC_BYTES + sizeof(KvBarriers);
+  return 1024 + (size_t)stages * (A_STAGE_BYTES + KV_B_STAGE_BYTES) + KV_STG_BYTES + KV_VEC_BYTES + KV_SLOT_BYTES + sizeof(KvBarriers);
 }
 int kv_pick_stages(int num_kb) {
-  const size_t budget = 232448 - 1024 - KV_STG_BYTES - KV_VEC_BYTES - sizeof(KvBarriers);
+  const size_t budget = 232448 - 1024 - KV_STG_BYTES - KV_VEC_BYTES - KV_SLOT_BYTES - sizeof(KvBarriers);
   int st = (int)(budget / (A_STAGE_BYTES + KV_B_STAGE_BYTES));
   if (st > MAX_STAGES) st = MAX_STAGES;
   if (st > 2 * num_kb) st = 2 * num_kb;
@@ -118,7 +120,9 @@ constexpr int KV_NTHREADS = (KV_FIRST_EPI_WARP + KV_EPI_WARPS) * 32;   // 640
 // DYN: dynamic tile scheduling (hybrid static share + claimed chunks) -- used where tiles are long (PATCH GEMM-3,
 // K = d_model) and SMs drift apart; the REUSE decode keeps the static split, whose epilogue has no registers
 // to spare for the scheduler state.
-template <bool DYN>
+// SCALED: rows carry a scale (e4m3 code scales and / or the RMS scale of PATCH GEMM-3); REUSE decode of bf16 codes
+// compiles it out (no per-tile scale fetch, mean added with one packed add).
+template <bool DYN, bool SCALED>
 __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -127,7 +131,8 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
   uint8_t* smem_stg = smem_b + STAGES * KV_B_STAGE_BYTES;
   uint8_t* smem_vec = smem_stg + KV_STG_BYTES;
-  KvBarriers* bars = (KvBarriers*)(smem_vec + KV_VEC_BYTES);
+  uint8_t* smem_slot = smem_vec + KV_VEC_BYTES;
+  KvBarriers* bars = (KvBarriers*)(smem_slot + KV_SLOT_BYTES);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.m_tiles * P.n_segs * P.n_tiles;
@@ -276,14 +281,19 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
     ptx::setmaxnreg_inc<112>();
     const int q = warp & 3;                                   // TMEM lane quadrant this warp may read
     const int g = (warp - KV_FIRST_EPI_WARP) >> 2;            // frequency / column group 0..3
-    const uint32_t stg = ptx::smem_u32(smem_stg) + (uint32_t)q * (32 * 512);
+    const uint32_t stg = ptx::smem_u32(smem_stg) + (uint32_t)q * (32 * KV_ROW_PITCH);
     const uint32_t wvec = ptx::smem_u32(smem_vec) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 256;
+    // the quadrant's 32 slot numbers, one private copy per warp (no cross-warp ordering needed): the copy-out reads the
+    // slot of the row it stores with one broadcast LDS instead of shuffling a 64-bit address out of the owning lane
+    const uint32_t wslot = ptx::smem_u32(smem_slot) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 128;
     const uint32_t bar_id = 1 + q;
+    const uint32_t row_stride = (uint32_t)P.pool_width * 2u;  // bytes per slot
+    // this lane's float4 of the warp's mean / bias slice: tile column for K tiles (runs a | b of both heads) / V tiles
+    const int vcol_k = ((lane >> 3) & 1) * 128 + ((lane >> 2) & 1) * 64 + 16 * g + (lane & 3) * 4;
+    const int vcol_v = 64 * g + lane * 4;
 
     // per-row state, recomputed when the m-tile changes (DYN: or the segment -- the RMS scale belongs to a layer)
     int cur_m = -1, cur_seg = -1;
-    unsigned long long slot_off = 0;                          // byte offset of the row's slot inside a pool
-    bool valid = false;
     float rs_row = 1.0f;
     unsigned long long c2[8], s2[8];                          // (cos, sin) of frequencies 16g + {2i, 2i+1}, packed pairs
 #pragma unroll
@@ -300,12 +310,8 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       pr.a_scale = 1.0f;
       const TcSeg& sg = P.segs[tc.seg];
       const int n0 = tc.n_tile * KV_BLOCK_N;
-      if (sg.col_vec && lane < 16) {
-        const int run = lane >> 2, part = lane & 3;
-        const int col = (n0 < sg.rope_cols) ? (run >> 1) * 128 + (run & 1) * 64 + 16 * g + part * 4 : 64 * g + lane * 4;
-        pr.vec = ldg_f4(sg.col_vec + n0 + col);
-      }
-      if (sg.a_scale) {
+      if (sg.col_vec && lane < 16) pr.vec = ldg_f4(sg.col_vec + n0 + ((n0 < sg.rope_cols) ? vcol_k : vcol_v));
+      if (SCALED && sg.a_scale) {
         const int row = tc.m_tile * BLOCK_M + q * 32 + lane;
         if (row < P.M) pr.a_scale = __ldg(sg.a_scale + row);
       }
@@ -344,20 +350,20 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         cur_m = tc.m_tile;
         cur_seg = tc.seg;
         const int row = cur_m * BLOCK_M + q * 32 + lane;
-        valid = row < P.M;
         int pos = 0;
-        long long slot = 0;
+        long long slot = -1;                                    // stays -1 for rows beyond M and page ids outside the pool
         rs_row = 1.0f;
-        if (valid) {
+        if (row < P.M) {
           row_to_pos_slot(P.batch, row, pos, slot);
-          valid = slot >= 0;                                    // -1: page id outside the pool -> the row is not written
-          if (sg.rowscale_in) {                                 // NORM_RMS (PATCH GEMM-3; several segments only with DYN)
+          if (SCALED && sg.rowscale_in) {                       // NORM_RMS (PATCH GEMM-3; several segments only with DYN)
             float ss = 0.0f;
             for (int p = 0; p < P.n_partials; ++p) ss += __ldg(sg.rowscale_in + (size_t)p * P.M + row);
             rs_row = rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
           }
         }
-        slot_off = (unsigned long long)slot * (unsigned long long)P.pool_width * 2ull;
+        __syncwarp();
+        asm volatile("st.shared.b32 [%0], %1;" ::"r"(wslot + lane * 4), "r"((int)slot) : "memory");
+        __syncwarp();
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           const float2 x = rope_cs(pos, P.rope_g[16 * g + 2 * i]), y = rope_cs(pos, P.rope_g[16 * g + 2 * i + 1]);
@@ -368,9 +374,9 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       const float rs = rs_row * cur.a_scale;
       const unsigned long long rs2 = f2_pack(rs, rs);
       const bool to1 = n0 >= P.split;
-      const unsigned long long row_base =
-          valid ? (unsigned long long)(to1 ? sg.out1 : sg.out0) + slot_off + (unsigned long long)(to1 ? n0 - P.split : n0) * 2ull
-                : 0ull;
+      // address of this lane's 16 bytes in slot 0 of the tile's pool columns; a row adds slot * row_stride
+      const unsigned long long tile_base = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
+                                           (unsigned long long)(to1 ? n0 - P.split : n0) * 2ull + (unsigned long long)lane * 16ull;
 
       // this warp's slice of the tile's mean / bias: wvec[16 * run + i]
       __syncwarp();
@@ -403,10 +409,12 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
               const int i = q4 * 4 + e * 2, k = q4 * 2 + e;
-              const unsigned long long a = f2_fma(f2_pack(__uint_as_float(ra[i]), __uint_as_float(ra[i + 1])), rs2,
-                                                  e ? f2_pack(ma.z, ma.w) : f2_pack(ma.x, ma.y));
-              const unsigned long long b = f2_fma(f2_pack(__uint_as_float(rb[i]), __uint_as_float(rb[i + 1])), rs2,
-                                                  e ? f2_pack(mb.z, mb.w) : f2_pack(mb.x, mb.y));
+              const unsigned long long am = e ? f2_pack(ma.z, ma.w) : f2_pack(ma.x, ma.y);
+              const unsigned long long bm = e ? f2_pack(mb.z, mb.w) : f2_pack(mb.x, mb.y);
+              const unsigned long long av = f2_pack(__uint_as_float(ra[i]), __uint_as_float(ra[i + 1]));
+              const unsigned long long bv = f2_pack(__uint_as_float(rb[i]), __uint_as_float(rb[i + 1]));
+              const unsigned long long a = SCALED ? f2_fma(av, rs2, am) : f2_add(av, am);
+              const unsigned long long b = SCALED ? f2_fma(bv, rs2, bm) : f2_add(bv, bm);
               float x0, x1, y0, y1, t0, t1;
               f2_unpack(f2_mul(b, s2[k]), t0, t1);
               f2_unpack(f2_fma(a, c2[k], f2_pack(-t0, -t1)), x0, x1);     // a cos - b sin
@@ -434,8 +442,10 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
           for (int q4 = 0; q4 < 8; ++q4) {
             const float4 m4 = ptx::lds_f4(wvec + (c * 32 + q4 * 4) * 4);
             float v0, v1, v2, v3;
-            f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q4 * 4]), __uint_as_float(r[q4 * 4 + 1])), rs2, f2_pack(m4.x, m4.y)), v0, v1);
-            f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q4 * 4 + 2]), __uint_as_float(r[q4 * 4 + 3])), rs2, f2_pack(m4.z, m4.w)), v2, v3);
+            const unsigned long long r01 = f2_pack(__uint_as_float(r[q4 * 4]), __uint_as_float(r[q4 * 4 + 1]));
+            const unsigned long long r23 = f2_pack(__uint_as_float(r[q4 * 4 + 2]), __uint_as_float(r[q4 * 4 + 3]));
+            f2_unpack(SCALED ? f2_fma(r01, rs2, f2_pack(m4.x, m4.y)) : f2_add(r01, f2_pack(m4.x, m4.y)), v0, v1);
+            f2_unpack(SCALED ? f2_fma(r23, rs2, f2_pack(m4.z, m4.w)) : f2_add(r23, f2_pack(m4.z, m4.w)), v2, v3);
             o[q4 * 2] = pack_bf16x2(v0, v1);
             o[q4 * 2 + 1] = pack_bf16x2(v2, v3);
           }
@@ -452,16 +462,16 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       if (g == 0 && lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
       {
         uint4 v[8];
-        unsigned long long base[8];
+        int sl[8];
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           const int r = 8 * g + i;
-          base[i] = __shfl_sync(0xffffffffu, row_base, r);
+          asm volatile("ld.shared.b32 %0, [%1];" : "=r"(sl[i]) : "r"(wslot + r * 4) : "memory");
           v[i] = ptx::lds128(qstg_addr(stg, r, lane));
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i)
-          if (base[i] != 0ull) ptx::stg128_cs(base[i] + (unsigned long long)lane * 16ull, v[i]);
+          if (sl[i] >= 0) ptx::stg128_cs(tile_base + (unsigned long long)(uint32_t)sl[i] * row_stride, v[i]);
       }
       cur = nxt;
       tc = tn;
@@ -497,16 +507,21 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   const size_t smem = kv_smem_bytes(P.stages);
   static std::atomic<size_t> configured[SCD_MAX_DEVICES];      // the attribute belongs to (function, device)
   if (configured[p->device].load(std::memory_order_relaxed) < smem) {
-    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
     configured[p->device].store(smem, std::memory_order_relaxed);
   }
   const int grid = std::min(total, p->sm_count);
   // long tiles (K = d_model: PATCH GEMM-3): KV_STATIC_PCT % of an even split is owned statically, the rest is
   // claimed tile by tile; short tiles (REUSE decode): static split only
-  bool multi_rowscale = false;                              // several layers' RMS scales: only the DYN variant tracks the segment
-  for (int i = 0; i < P.n_segs; ++i) multi_rowscale |= P.n_segs > 1 && P.segs[i].rowscale_in != nullptr;
+  bool multi_rowscale = false, scaled = false;              // several layers' RMS scales: only the DYN variant tracks the segment
+  for (int i = 0; i < P.n_segs; ++i) {
+    multi_rowscale |= P.n_segs > 1 && P.segs[i].rowscale_in != nullptr;
+    scaled |= P.segs[i].rowscale_in != nullptr || P.segs[i].a_scale != nullptr;
+  }
+  if ((long long)P.pool_slots >= (1ll << 31)) return fail(SCD_E_UNSUPPORTED, "pools of more than 2^31 slots");
   const bool dyn = (P.num_kb >= 16 && total > grid) || multi_rowscale;
   prof_begin(s);
   if (dyn) {
@@ -515,9 +530,11 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
     P.dyn_begin = grid * P.static_tiles;
     P.n_chunks = total - P.dyn_begin;
     P.sched = p->kv_sched + 2 * (p->kv_sched_next.fetch_add(1) % KV_SCHED_SETS);
-    launch_pdl(tc_kv_kernel<true>, grid, KV_NTHREADS, smem, s, P);
+    launch_pdl(tc_kv_kernel<true, true>, grid, KV_NTHREADS, smem, s, P);
+  } else if (scaled) {
+    launch_pdl(tc_kv_kernel<false, true>, grid, KV_NTHREADS, smem, s, P);
   } else {
-    launch_pdl(tc_kv_kernel<false>, grid, KV_NTHREADS, smem, s, P);
+    launch_pdl(tc_kv_kernel<false, false>, grid, KV_NTHREADS, smem, s, P);
   }
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
