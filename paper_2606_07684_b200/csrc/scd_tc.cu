@@ -964,7 +964,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   }
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
-  launch_pdl(tc_gemm_kernel<EPI, AMODE>, grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, smem, s, P);
+  launch_pdl(tc_gemm_kernel<EPI, AMODE>, grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, smem, s, 1, P);
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));

@@ -530,11 +530,11 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
     P.dyn_begin = grid * P.static_tiles;
     P.n_chunks = total - P.dyn_begin;
     P.sched = p->kv_sched + 2 * (p->kv_sched_next.fetch_add(1) % KV_SCHED_SETS);
-    launch_pdl(tc_kv_kernel<true, true>, grid, KV_NTHREADS, smem, s, P);
+    launch_pdl(tc_kv_kernel<true, true>, grid, KV_NTHREADS, smem, s, 1, P);
   } else if (scaled) {
-    launch_pdl(tc_kv_kernel<false, true>, grid, KV_NTHREADS, smem, s, P);
+    launch_pdl(tc_kv_kernel<false, true>, grid, KV_NTHREADS, smem, s, 1, P);
   } else {
-    launch_pdl(tc_kv_kernel<false, false>, grid, KV_NTHREADS, smem, s, P);
+    launch_pdl(tc_kv_kernel<false, false>, grid, KV_NTHREADS, smem, s, 1, P);
   }
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
