@@ -88,14 +88,6 @@ __device__ __forceinline__ void tile_decode(const TcParams& P, int tile, int& m_
   m_tile = sb * P.msb + (rem - n_tile * rows);
 }
 
-// two e4m3 codes, each in the high byte of a 16-bit half -> two bf16 (exact)
-__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t x) {
-  const uint32_t y = (x & 0x80008000u) | ((x >> 4) & 0x07f007f0u);
-  uint32_t r;
-  asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(y), "r"(0x7b807b80u));   // x 2^120
-  return r;
-}
-
 // per-warp staging tile (shared-space address `stg`): row pitch `pitch` bytes (>= 128), 16-byte
 // chunks XOR-swizzled on the low 3 bits of the row so that row-per-thread writes and
 // row-per-half-warp reads are both bank-conflict free
@@ -1134,8 +1126,11 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
     }
     P.prof_id = SCD_PROF_REUSE_DECODE;
     P.head_rank = m.reuse_per_head ? s0.rank / m.n_kv_heads : 0;
-    if (e4) st = launch_tc<EPI_KV, A_CODES>(p, P, s);       // operand expansion in shared memory (generic kernel)
-    else st = tc_kv_eligible(p, P) ? launch_tc_kv(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
+    P.a_is_codes = 1;
+    // the paged-KV kernel takes 256-column tiles of 128-wide heads (e4m3 codes: widened in shared memory by its own
+    // warps); anything else runs on the generic kernel
+    if (tc_kv_eligible(p, P)) st = launch_tc_kv(p, P, s);
+    else st = e4 ? launch_tc<EPI_KV, A_CODES>(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
     if (st != SCD_OK) return st;
     i = j;
   }

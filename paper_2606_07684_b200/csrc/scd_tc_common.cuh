@@ -47,6 +47,7 @@ struct TcParams {
   int32_t head_rank;                  // paged-KV kernel, per-head REUSE: codes per head (A/B are block-diagonal), else 0
   int32_t prof_id;                    // host only: id under which scd_profile_* reports the launch
   int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
+  int32_t a_is_codes;                 // paged-KV kernel: A is a code segment (e4m3 codes are widened in shared memory)
   long long pool_slots;               // paged epilogues: n_blocks * block_size (slot numbers are kept as int32)
 };
 
@@ -71,6 +72,15 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 __device__ __forceinline__ float2 rope_cs(int pos, uint32_t g) {
   const float x = (float)(int32_t)((uint32_t)pos * g) * 1.4629180792671596e-9f;   // 2 pi / 2^32
   return make_float2(__cosf(x), __sinf(x));
+}
+
+// two e4m3 codes, each in the high byte of a 16-bit half -> two bf16 (exact): s.eeee.mmm -> s.0000eeee.mmm0000 is the
+// same number times 2^-120, normals and subnormals alike; one exact bf16 multiply by 2^120 finishes the conversion
+__device__ __forceinline__ uint32_t e4m3x2_to_bf16x2(uint32_t x) {
+  const uint32_t y = (x & 0x80008000u) | ((x >> 4) & 0x07f007f0u);
+  uint32_t r;
+  asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(r) : "r"(y), "r"(0x7b807b80u));   // x 2^120
+  return r;
 }
 
 // packed fp32 pairs (FFMA2 / FMUL2 on sm_100a): half the FMA-pipe instructions of the epilogue

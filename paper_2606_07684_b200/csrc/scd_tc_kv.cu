@@ -36,7 +36,7 @@ constexpr int KV_VEC_BYTES = KV_EPI_WARPS * 64 * 4;          // per-warp slice o
 constexpr int KV_SLOT_BYTES = KV_EPI_WARPS * 32 * 4;         // per-warp copy of its quadrant's 32 slot numbers (-1 = no row)
 
 struct __align__(8) KvBarriers {
-  uint64_t full[MAX_STAGES], empty[MAX_STAGES];
+  uint64_t full[MAX_STAGES], empty[MAX_STAGES], ready[MAX_STAGES];
   uint64_t tmem_full[2], tmem_empty[2];
   uint64_t sched_full[4], sched_empty[4];                    // chunk ring (KV_SCHED_SLOTS)
   int32_t sched_begin[4], sched_end[4];                      // tile range of the entry; begin < 0 = no more work
@@ -116,14 +116,21 @@ __device__ __forceinline__ TileCoord tile_coord(const TcParams& P, int tile) {
 // ---------------------------------------------------------------------------------
 constexpr int KV_FIRST_EPI_WARP = 4;
 constexpr int KV_NTHREADS = (KV_FIRST_EPI_WARP + KV_EPI_WARPS) * 32;   // 640
+constexpr int KV_XF_WARPS = 4;                                          // AE4: one code-widening warp per SM sub-partition
+constexpr int KV_NTHREADS_E4 = KV_NTHREADS + KV_XF_WARPS * 32;          // 768
 
 // DYN: dynamic tile scheduling (hybrid static share + claimed chunks) -- used where tiles are long (PATCH GEMM-3,
 // K = d_model) and SMs drift apart; the REUSE decode keeps the static split, whose epilogue has no registers
 // to spare for the scheduler state.
 // SCALED: rows carry a scale (e4m3 code scales and / or the RMS scale of PATCH GEMM-3); REUSE decode of bf16 codes
 // compiles it out (no per-tile scale fetch, mean added with one packed add).
-template <bool DYN, bool SCALED>
-__global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
+// AE4: the A operand is a segment of e4m3 codes (config 4).  tcgen05 has no bf16 x fp8 MMA and the basis must stay bf16,
+// so the raw tile [128 rows x 64 B] lands in the upper half of the A stage and four extra warps (24 in all; registers
+// re-dealt 24 / 104 / 40) widen it in place to the swizzled bf16 tile before the MMA may read it -- exactly (all 254
+// finite codes, test_e4m3_operand_expansion_is_exact_for_every_code); the row scale is applied in the epilogue.
+template <bool DYN, bool SCALED, bool AE4>
+__global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
+  static_assert(!AE4 || (SCALED && !DYN), "e4m3 codes carry row scales; static split");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
@@ -144,6 +151,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
     for (int s = 0; s < STAGES; ++s) {
       ptx::mbar_init(&bars->full[s], 1);
       ptx::mbar_init(&bars->empty[s], 1);
+      ptx::mbar_init(&bars->ready[s], KV_XF_WARPS * 32);
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
@@ -167,7 +175,9 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
   ptx::grid_dep_launch_dependents();    // the next one may start its prologue as SMs free up
 
   if (warp < KV_FIRST_EPI_WARP) {
-    ptx::setmaxnreg_dec<32>();   // 128 x 32 + 512 x 112 = 640 x 96: the CTA pool is what the launch allocated
+    // 128 x 32 + 512 x 112 = 640 x 96 (AE4: 128 x 24 + 512 x 104 + 128 x 40 = 768 x 80): the pool the launch allocated
+    if (AE4) ptx::setmaxnreg_dec<24>();
+    else ptx::setmaxnreg_dec<32>();
   if (warp == 0) {
     // ============================== TMA producer ==============================
     if (lane == 0) {
@@ -210,9 +220,9 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         tile_kb_range(P, tc.n_tile, kb0, kb1);
         for (int kb = kb0; kb < kb1; ++kb) {
           ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
-          ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES + KV_B_STAGE_BYTES);
-          ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES, am, &bars->full[stage], kb * BLOCK_K, tc.m_tile * BLOCK_M,
-                           sg.a_z);
+          ptx::mbar_expect_tx(&bars->full[stage], (AE4 ? A_STAGE_BYTES / 2 : A_STAGE_BYTES) + KV_B_STAGE_BYTES);
+          ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES + (AE4 ? A_STAGE_BYTES / 2 : 0), am, &bars->full[stage], kb * BLOCK_K,
+                           tc.m_tile * BLOCK_M, sg.a_z);
           ptx::tma_load_2d(smem_b + stage * KV_B_STAGE_BYTES, bm, &bars->full[stage], kb * BLOCK_K,
                            tc.n_tile * KV_BLOCK_N);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
@@ -261,7 +271,7 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
         tile_kb_range(P, n_tile, kb0, kb1);
         if (++n_tile == P.n_tiles) n_tile = 0;
         for (int kb = kb0; kb < kb1; ++kb) {
-          ptx::mbar_wait_suspend(&bars->full[stage], phase);
+          ptx::mbar_wait_suspend(AE4 ? &bars->ready[stage] : &bars->full[stage], phase);   // ready: landed and widened
           ptx::tc_fence_after();
           const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
           const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * KV_B_STAGE_BYTES));
@@ -276,9 +286,51 @@ __global__ void __launch_bounds__(KV_NTHREADS, 1) tc_kv_kernel(const __grid_cons
       }
     }
   }
+  } else if (AE4 && warp >= KV_FIRST_EPI_WARP + KV_EPI_WARPS) {
+    // ============================== A transform: e4m3 -> bf16 in shared memory ==============================
+    // 512 items of 16 codes per k-block (row = item / 4, quarter = item % 4), four per thread, read conflict-free from
+    // the raw tile in bytes [8192, 16384) of the stage; all 128 threads meet (the widened rows overwrite the raw
+    // bytes); then each item becomes chunks 2 quarter, 2 quarter + 1 of its row in the 128-byte-swizzled K-major layout.
+    ptx::setmaxnreg_dec<40>();
+    const int xt = threadIdx.x - (KV_FIRST_EPI_WARP + KV_EPI_WARPS) * 32;
+    const uint32_t a_base = ptx::smem_u32(smem_a);
+    int stage = 0;
+    uint32_t phase = 0;
+    int n_tile = s_begin % P.n_tiles;
+    for (int tile = s_begin; tile < s_end; ++tile) {
+      int kb0, kb1;
+      tile_kb_range(P, n_tile, kb0, kb1);
+      if (++n_tile == P.n_tiles) n_tile = 0;
+      for (int kb = kb0; kb < kb1; ++kb) {
+        ptx::mbar_wait_suspend(&bars->full[stage], phase);
+        const uint32_t sb = a_base + (uint32_t)stage * A_STAGE_BYTES;
+        uint4 raw[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) raw[j] = ptx::lds128(sb + A_STAGE_BYTES / 2 + (uint32_t)(xt + 128 * j) * 16);
+        ptx::named_bar_sync(5, KV_XF_WARPS * 32);
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const int item = xt + 128 * j, row = item >> 2, qt = item & 3;
+          const uint32_t row_off = (uint32_t)(row >> 3) * 1024 + (uint32_t)(row & 7) * 128;
+          const uint32_t w[4] = {raw[j].x, raw[j].y, raw[j].z, raw[j].w};
+          uint32_t o[8];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            o[2 * i] = e4m3x2_to_bf16x2(__byte_perm(w[i], 0u, 0x1404));       // bytes 0, 1 -> high bytes of two halves
+            o[2 * i + 1] = e4m3x2_to_bf16x2(__byte_perm(w[i], 0u, 0x3424));   // bytes 2, 3
+          }
+          ptx::sts128(sb + row_off + (uint32_t)(((2 * qt) ^ (row & 7)) << 4), make_uint4(o[0], o[1], o[2], o[3]));
+          ptx::sts128(sb + row_off + (uint32_t)(((2 * qt + 1) ^ (row & 7)) << 4), make_uint4(o[4], o[5], o[6], o[7]));
+        }
+        ptx::fence_proxy_async_smem();
+        ptx::mbar_arrive(&bars->ready[stage]);
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+      }
+    }
   } else {
     // ============================== epilogue ==============================
-    ptx::setmaxnreg_inc<112>();
+    if (AE4) ptx::setmaxnreg_inc<104>();
+    else ptx::setmaxnreg_inc<112>();
     const int q = warp & 3;                                   // TMEM lane quadrant this warp may read
     const int g = (warp - KV_FIRST_EPI_WARP) >> 2;            // frequency / column group 0..3
     const uint32_t stg = ptx::smem_u32(smem_stg) + (uint32_t)q * (32 * KV_ROW_PITCH);
@@ -507,9 +559,10 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   const size_t smem = kv_smem_bytes(P.stages);
   static std::atomic<size_t> configured[SCD_MAX_DEVICES];      // the attribute belongs to (function, device)
   if (configured[p->device].load(std::memory_order_relaxed) < smem) {
-    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
     configured[p->device].store(smem, std::memory_order_relaxed);
   }
@@ -523,18 +576,22 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   }
   if ((long long)P.pool_slots >= (1ll << 31)) return fail(SCD_E_UNSUPPORTED, "pools of more than 2^31 slots");
   const bool dyn = (P.num_kb >= 16 && total > grid) || multi_rowscale;
+  const bool ae4 = P.code_dtype == SCD_E4M3_ROWSCALE && P.a_is_codes;
+  if (ae4 && dyn) return fail(SCD_E_UNSUPPORTED, "internal: e4m3 codes on the dynamically scheduled paged-KV kernel");
   prof_begin(s);
-  if (dyn) {
+  if (ae4) {
+    launch_pdl(tc_kv_kernel<false, true, true>, grid, KV_NTHREADS_E4, smem, s, 1, P);
+  } else if (dyn) {
     P.chunk_tiles = 1;
     P.static_tiles = (int)((long long)total * KV_STATIC_PCT / 100 / grid);
     P.dyn_begin = grid * P.static_tiles;
     P.n_chunks = total - P.dyn_begin;
     P.sched = p->kv_sched + 2 * (p->kv_sched_next.fetch_add(1) % KV_SCHED_SETS);
-    launch_pdl(tc_kv_kernel<true, true>, grid, KV_NTHREADS, smem, s, 1, P);
+    launch_pdl(tc_kv_kernel<true, true, false>, grid, KV_NTHREADS, smem, s, 1, P);
   } else if (scaled) {
-    launch_pdl(tc_kv_kernel<false, true>, grid, KV_NTHREADS, smem, s, 1, P);
+    launch_pdl(tc_kv_kernel<false, true, false>, grid, KV_NTHREADS, smem, s, 1, P);
   } else {
-    launch_pdl(tc_kv_kernel<false, false>, grid, KV_NTHREADS, smem, s, 1, P);
+    launch_pdl(tc_kv_kernel<false, false, false>, grid, KV_NTHREADS, smem, s, 1, P);
   }
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
