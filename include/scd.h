@@ -204,6 +204,44 @@ scd_status_t scd_patch_layers(const scd_plan_t* plan, const scd_batch_t* batch, 
                               const scd_paged_kv_t* kv, void* workspace, size_t workspace_bytes,
                               int32_t layer_begin, int32_t layer_end, void* stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Group-wise INT4 KV codec -- the paper's fastest transport baseline ("Quantized KV: transmits 4-bit
+ * quantized KV caches (group-wise INT4) and dequantizes on the consumer"; Table 4
+ * :352-359), built as the same-box comparison codec.  The paper fixes neither group
+ * size nor range convention; reading (U19): a group is `group` consecutive channels
+ * of one token row (32, 64 or 128, dividing head_dim), lo = min, hi = max of the group,
+ * s = bf16((hi - lo) / 15) (1 if that is 0), q = clamp(rint((x - lo) / s), 0, 15), all in IEEE fp32;
+ * byte j of a row = q[2j] | q[2j+1] << 4; metadata per group = bf16 s and bf16 lo;
+ * dequantised x^ = bf16(q * s + lo).  Bit-exact against oracle/int4_oracle.py.
+ *
+ * Packed buffer (DEVICE, 128-byte aligned, caller owned): tensor i at i * tensor_stride holds the nibbles
+ * [T, W/2] at 0, the scales [T, W/group] bf16 at scale_offset and the zero points [T, W/group] bf16 at
+ * zero_offset (W = n_kv_heads * head_dim).  A "tensor" is one layer's K or V; the caller chooses the order.
+ * Both calls enqueue on `stream` and return; no allocation, no synchronisation; statuses as above.
+ * --------------------------------------------------------------------------------------------- */
+typedef struct {
+  int32_t n_kv_heads, head_dim, block_size, group;
+} scd_int4_desc_t;
+
+/* Layout arithmetic (pure host).  payload_bytes = |Z| of Eq. 3: nibbles + metadata, no padding.
+ * Any out pointer may be NULL. */
+scd_status_t scd_int4_layout(const scd_int4_desc_t* desc, int32_t total_tokens, int32_t n_tensors,
+                             size_t* tensor_stride, size_t* scale_offset, size_t* zero_offset,
+                             size_t* total_bytes, size_t* payload_bytes);
+
+/* Producer: src = HOST array of n_tensors DEVICE pointers -> [total_tokens, H_kv, d_h] bf16 with dense heads
+ * and `token_stride` elements between token rows (multiple of 8, >= W); writes every tensor's segment of
+ * `packed`. */
+scd_status_t scd_int4_quantize(const scd_int4_desc_t* desc, int32_t total_tokens, int32_t n_tensors,
+                               const void* const* src, int64_t token_stride, void* packed, void* stream);
+
+/* Consumer: dequantises tensor i into pools[i] (HOST array of DEVICE pointers ->
+ * [n_blocks, block_size, H_kv, d_h] bf16) at slot = page_table[b][t / bs] * bs + t % bs; slots outside the
+ * batch are not written; a page id outside [0, n_blocks) skips the token.  pos_offset is not used. */
+scd_status_t scd_int4_dequantize_paged(const scd_int4_desc_t* desc, const scd_batch_t* batch, int32_t n_tensors,
+                                       const void* packed, void* const* pools, int32_t n_blocks, void* stream);
+
+
 /* Number of kernels the last hot call on this thread enqueued (for bench accounting). */
 int32_t scd_last_launch_count(void);
 

@@ -33,7 +33,8 @@ NO_SCALE = C.c_size_t(-1).value
 EXPORTS = ["scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
            "scd_encode", "scd_reuse_decode", "scd_patch", "scd_encode_layers", "scd_reuse_decode_layers",
            "scd_patch_layers", "scd_last_launch_count", "scd_profile_enable",
-           "scd_profile_fetch", "scd_last_error", "scd_version"]
+           "scd_profile_fetch", "scd_last_error", "scd_version",
+           "scd_int4_layout", "scd_int4_quantize", "scd_int4_dequantize_paged"]
 
 
 class ModelDesc(C.Structure):
@@ -72,6 +73,10 @@ class PagedKV(C.Structure):
     _fields_ = [("k_pool", C.POINTER(C.c_void_p)), ("v_pool", C.POINTER(C.c_void_p)), ("n_blocks", C.c_int32)]
 
 
+class Int4Desc(C.Structure):
+    _fields_ = [("n_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("block_size", C.c_int32), ("group", C.c_int32)]
+
+
 class ScdError(RuntimeError):
     def __init__(self, status: int, msg: str):
         super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
@@ -98,6 +103,11 @@ def _load() -> C.CDLL:
     lib.scd_patch_layers.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), vp, sz, i32, i32, vp]
     for name in ("scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
                  "scd_encode", "scd_reuse_decode", "scd_patch"):
+        getattr(lib, name).restype = C.c_int
+    lib.scd_int4_layout.argtypes = [C.POINTER(Int4Desc), i32, i32, psz, psz, psz, psz, psz]
+    lib.scd_int4_quantize.argtypes = [C.POINTER(Int4Desc), i32, i32, C.POINTER(vp), C.c_int64, vp, vp]
+    lib.scd_int4_dequantize_paged.argtypes = [C.POINTER(Int4Desc), C.POINTER(BatchDesc), i32, vp, C.POINTER(vp), i32, vp]
+    for name in ("scd_int4_layout", "scd_int4_quantize", "scd_int4_dequantize_paged"):
         getattr(lib, name).restype = C.c_int
     lib.scd_last_launch_count.restype = C.c_int32
     lib.scd_profile_enable.argtypes = [i32]
@@ -260,6 +270,27 @@ def scd_patch(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequenc
     else:
         _check(lib.scd_patch_layers(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _ptr(workspace), ws_bytes,
                                     layers[0], layers[1], _stream_ptr(stream)))
+    return lib.scd_last_launch_count()
+
+
+def scd_int4_layout(desc: Int4Desc, total_tokens: int, n_tensors: int):
+    """(tensor_stride, scale_offset, zero_offset, total_bytes, payload_bytes); pure host arithmetic."""
+    v = [C.c_size_t(0) for _ in range(5)]
+    _check(lib.scd_int4_layout(C.byref(desc), total_tokens, n_tensors, *[C.byref(x) for x in v]))
+    return tuple(x.value for x in v)
+
+
+def scd_int4_quantize(desc: Int4Desc, total_tokens: int, src: Sequence[torch.Tensor], token_stride: int,
+                      packed: torch.Tensor, stream=None) -> int:
+    _check(lib.scd_int4_quantize(C.byref(desc), total_tokens, len(src), _ptr_array(src), token_stride, _ptr(packed),
+                                 _stream_ptr(stream)))
+    return lib.scd_last_launch_count()
+
+
+def scd_int4_dequantize_paged(desc: Int4Desc, batch: BatchDesc, packed: torch.Tensor, pools: Sequence[torch.Tensor],
+                              n_blocks: int, stream=None) -> int:
+    _check(lib.scd_int4_dequantize_paged(C.byref(desc), C.byref(batch), len(pools), _ptr(packed), _ptr_array(pools),
+                                         n_blocks, _stream_ptr(stream)))
     return lib.scd_last_launch_count()
 
 

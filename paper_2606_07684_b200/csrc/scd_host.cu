@@ -23,6 +23,7 @@ scd_status_t fail(scd_status_t st, const char* fmt, ...) {
   return st;
 }
 void count_launch() { ++g_launches; }
+void reset_launch_count() { g_launches = 0; }
 static thread_local int g_layer_begin = 0, g_layer_end = 1 << 30;
 bool layer_in_window(int layer) { return layer >= g_layer_begin && layer < g_layer_end; }
 struct LayerWindow {                       // scoped: set by the *_layers entry points

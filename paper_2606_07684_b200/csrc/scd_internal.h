@@ -31,7 +31,7 @@ enum EpiKind : int {
 // ids under which scd_profile_fetch reports the launches of the tensor-core path
 enum ProfId : int {
   SCD_PROF_ENCODE = 100, SCD_PROF_ENCODE_K = 101, SCD_PROF_REUSE_DECODE = 110, SCD_PROF_PATCH_GEMM1 = 120,
-  SCD_PROF_PATCH_GEMM2 = 130, SCD_PROF_PATCH_GEMM3 = 140
+  SCD_PROF_PATCH_GEMM2 = 130, SCD_PROF_PATCH_GEMM3 = 140, SCD_PROF_INT4_QUANT = 200, SCD_PROF_INT4_DEQUANT = 201
 };
 
 enum AMode : int {
@@ -133,6 +133,7 @@ namespace scd {
 // ---- error plumbing (scd_host.cu) -------------------------------------------------
 scd_status_t fail(scd_status_t st, const char* fmt, ...);
 void count_launch();
+void reset_launch_count();               // at the top of every hot call (scd_last_launch_count)
 // layer window of the running hot call: the *_layers entry points restrict a call to [layer_begin, layer_end)
 bool layer_in_window(int layer);
 // profiling hooks (scd_profile_enable): bracket one launch with events on `s`

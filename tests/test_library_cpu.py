@@ -24,7 +24,7 @@ def B():
 def test_exports_every_declared_symbol(B):
     hdr = open(os.path.join(ROOT, "include", "scd.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    declared = set(re.findall(r"\b(scd_[a-z_]+)\s*\(", hdr))
+    declared = set(re.findall(r"\b(scd_[a-z0-9_]+)\s*\(", hdr))
     assert declared == set(B.EXPORTS), declared ^ set(B.EXPORTS)
     for name in declared:
         assert hasattr(B.lib, name), name
@@ -150,3 +150,19 @@ def test_workload_generator_basis_is_a_pca_basis():
     # regenerating a row range gives the same bits
     y = W.make_state(cfg, 0, 1, 100, "cpu", row_offset=200)
     assert torch.equal(y, x[200:300])
+
+
+def test_int4_layout_matches_oracle_payload_and_rejects_bad_groups(B):
+    """scd_int4_layout (pure host): payload = oracle's |Z| for the INT4 codec (Eq. 3 :86); segments
+    disjoint and 128-B aligned; unsupported groups rejected."""
+    from oracle import int4_oracle as Q
+    for group in (32, 64, 128):
+        desc = B.Int4Desc(8, 128, 16, group)
+        for T, n in ((1000, 3), (1, 1), (8192, 64)):
+            stride, soff, zoff, total, payload = B.scd_int4_layout(desc, T, n)
+            assert payload == Q.payload_bytes(T, 1024, group, n)
+            assert stride % 128 == 0 and soff % 128 == 0 and zoff % 128 == 0 and total == stride * n
+            assert T * 512 <= soff and soff + T * (1024 // group) * 2 <= zoff and zoff + T * (1024 // group) * 2 <= stride
+    for bad in (B.Int4Desc(8, 128, 16, 16), B.Int4Desc(8, 64, 16, 128), B.Int4Desc(0, 128, 16, 32)):
+        with pytest.raises(B.ScdError):
+            B.scd_int4_layout(bad, 10, 1)
