@@ -210,13 +210,13 @@ scd_status_t scd_patch_layers(const scd_plan_t* plan, const scd_batch_t* batch, 
  * :352-359), built as the same-box comparison codec.  The paper fixes neither group
  * size nor range convention; reading (U19): a group is `group` consecutive channels
  * of one token row (32, 64 or 128, dividing head_dim), lo = min, hi = max of the group,
- * s = bf16((hi - lo) / 15) (1 if that is 0), q = clamp(rint((x - lo) / s), 0, 15), all in IEEE fp32;
- * byte j of a row = q[2j] | q[2j+1] << 4; metadata per group = bf16 s and bf16 lo;
+ * s = bf16((hi - lo) / 15) (1 if that is 0), q = clamp(rint((x - lo) * (1 / s)), 0, 15), all in IEEE fp32;
+ * byte j of a row = q[2j] | q[2j+1] << 4; metadata per group = {bf16 s, bf16 lo} (4 bytes);
  * dequantised x^ = bf16(q * s + lo).  Bit-exact against oracle/int4_oracle.py.
  *
  * Packed buffer (DEVICE, 128-byte aligned, caller owned): tensor i at i * tensor_stride holds the nibbles
- * [T, W/2] at 0, the scales [T, W/group] bf16 at scale_offset and the zero points [T, W/group] bf16 at
- * zero_offset (W = n_kv_heads * head_dim).  A "tensor" is one layer's K or V; the caller chooses the order.
+ * [T, W/2] at 0 and the metadata [T, W/group] x {bf16 scale, bf16 zero point} at meta_offset
+ * (W = n_kv_heads * head_dim).  A "tensor" is one layer's K or V; the caller chooses the order.
  * Both calls enqueue on `stream` and return; no allocation, no synchronisation; statuses as above.
  * --------------------------------------------------------------------------------------------- */
 typedef struct {
@@ -226,8 +226,7 @@ typedef struct {
 /* Layout arithmetic (pure host).  payload_bytes = |Z| of Eq. 3: nibbles + metadata, no padding.
  * Any out pointer may be NULL. */
 scd_status_t scd_int4_layout(const scd_int4_desc_t* desc, int32_t total_tokens, int32_t n_tensors,
-                             size_t* tensor_stride, size_t* scale_offset, size_t* zero_offset,
-                             size_t* total_bytes, size_t* payload_bytes);
+                             size_t* tensor_stride, size_t* meta_offset, size_t* total_bytes, size_t* payload_bytes);
 
 /* Producer: src = HOST array of n_tensors DEVICE pointers -> [total_tokens, H_kv, d_h] bf16 with dense heads
  * and `token_stride` elements between token rows (multiple of 8, >= W); writes every tensor's segment of
@@ -241,6 +240,35 @@ scd_status_t scd_int4_quantize(const scd_int4_desc_t* desc, int32_t total_tokens
 scd_status_t scd_int4_dequantize_paged(const scd_int4_desc_t* desc, const scd_batch_t* batch, int32_t n_tensors,
                                        const void* packed, void* const* pools, int32_t n_blocks, void* stream);
 
+
+/* ---------------------------------------------------------------------------------------------
+ * Offline REUSE calibration fit: "Layer-wise Stack-SVD with Ridge Regression"
+ * (section 4.3.1, Eq. 6-7; App. F.1 :583-586; Table 6 :602 "Reuse fitting").  For one
+ * (layer, branch): paired samples A (producer), B (consumer), both [n_rows, width] bf16 row-major with
+ * `row_stride` elements between rows (keys in content space, i.e. deRoPE'd, Eq. 5); X = [A B];
+ *   V_r   = top-`rank` right singular vectors of X (of X minus its column means when center != 0)
+ *   W_dec = V_r^T = [W_dec,A | W_dec,B]  ([rank, width] each; Eq. 6 with Z = X V_r, reading U4)
+ *   W_enc = (A^T A + lam I)^-1 A^T Z,  lam = lam_rel * trace(A^T A) / width      (Eq. 7, reading U4)
+ *   sigma = the top singular values; mu_a, mu_b = column means (center != 0; reading U2).
+ * V_r is unique only up to the sign of each direction: compare V_r V_r^T, sigma and W_enc W_dec, never entries.
+ * Outputs (DEVICE) are written in out_dtype (F32 or BF16; sigma and means always fp32); w_dec_a, sigma may be NULL.
+ * The per-head reading is width = head_dim with the heads flattened into n_rows.
+ * NOT a hot call: it enqueues on `stream` and SYNCHRONISES it once per Jacobi sweep (convergence test);
+ * sweeps (HOST [2], may be NULL) receives the sweeps of the joint and of the ridge eigen-solve (at most 60 each).  Workspace (DEVICE,
+ * 256-byte aligned, scd_fit_query bytes: the K-major copy of X dominates, 4 * width * n_rows bytes).
+ * width: multiple of 8, <= 1024; bf16 states only (else SCD_E_UNSUPPORTED).
+ * --------------------------------------------------------------------------------------------- */
+typedef struct {
+  int32_t width, rank, center;
+  float lam_rel;
+  scd_dtype_t state_dtype, out_dtype;
+} scd_fit_desc_t;
+
+scd_status_t scd_fit_query(const scd_fit_desc_t* desc, int64_t n_rows, size_t* workspace_bytes);
+scd_status_t scd_fit_reuse(const scd_fit_desc_t* desc, const void* a, const void* b, int64_t n_rows, int64_t row_stride,
+                           void* w_enc /* [width, rank] */, void* w_dec_a /* [rank, width] */, void* w_dec_b /* [rank, width] */,
+                           float* mu_a /* [width] */, float* mu_b /* [width] */, float* sigma /* [rank] */,
+                           void* workspace, size_t workspace_bytes, int32_t* sweeps, void* stream);
 
 /* Number of kernels the last hot call on this thread enqueued (for bench accounting). */
 int32_t scd_last_launch_count(void);

@@ -17,7 +17,7 @@ significant bits).  Codes, metadata and dequantised bf16 values are compared BIT
 
   lo = min_i x_i ; hi = max_i x_i                        (exact: inputs are bf16)
   s  = bf16_rne( (hi - lo) / 15 )        fp32 subtract, fp32 divide ; s = 1 if that is 0 (constant group)
-  q_i = clamp( rint( (x_i - lo) / s ), 0, 15 )           fp32 subtract, fp32 divide, RNE to integer
+  q_i = clamp( rint( (x_i - lo) * (1 / s) ), 0, 15 )     fp32 subtract; 1 / s one fp32 divide; fp32 multiply; RNE to integer
   byte j of a row = q_{2j} | q_{2j+1} << 4
   dequantise:  x^_i = bf16_rne( q_i * s + lo )           fp32
 
@@ -52,7 +52,8 @@ def quantize(x: np.ndarray, group: int) -> Tuple[np.ndarray, np.ndarray, np.ndar
     hi = xg.max(axis=2)
     s = bf16_rne_f32((hi - lo).astype(np.float32) / np.float32(LEVELS))
     s = np.where(s == 0, np.float32(1.0), s).astype(np.float32)
-    t = (xg - lo[:, :, None]).astype(np.float32) / s[:, :, None]
+    inv = (np.float32(1.0) / s).astype(np.float32)
+    t = ((xg - lo[:, :, None]).astype(np.float32) * inv[:, :, None]).astype(np.float32)
     q = np.clip(np.rint(t), 0, LEVELS).astype(np.uint8).reshape(T, W)
     packed = (q[:, 0::2] | (q[:, 1::2] << 4)).astype(np.uint8)
     return q, packed, s, lo.astype(np.float32)

@@ -34,7 +34,8 @@ EXPORTS = ["scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segm
            "scd_encode", "scd_reuse_decode", "scd_patch", "scd_encode_layers", "scd_reuse_decode_layers",
            "scd_patch_layers", "scd_last_launch_count", "scd_profile_enable",
            "scd_profile_fetch", "scd_last_error", "scd_version",
-           "scd_int4_layout", "scd_int4_quantize", "scd_int4_dequantize_paged"]
+           "scd_int4_layout", "scd_int4_quantize", "scd_int4_dequantize_paged",
+           "scd_fit_query", "scd_fit_reuse"]
 
 
 class ModelDesc(C.Structure):
@@ -77,6 +78,11 @@ class Int4Desc(C.Structure):
     _fields_ = [("n_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("block_size", C.c_int32), ("group", C.c_int32)]
 
 
+class FitDesc(C.Structure):
+    _fields_ = [("width", C.c_int32), ("rank", C.c_int32), ("center", C.c_int32), ("lam_rel", C.c_float),
+                ("state_dtype", C.c_int32), ("out_dtype", C.c_int32)]
+
+
 class ScdError(RuntimeError):
     def __init__(self, status: int, msg: str):
         super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
@@ -104,11 +110,15 @@ def _load() -> C.CDLL:
     for name in ("scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
                  "scd_encode", "scd_reuse_decode", "scd_patch"):
         getattr(lib, name).restype = C.c_int
-    lib.scd_int4_layout.argtypes = [C.POINTER(Int4Desc), i32, i32, psz, psz, psz, psz, psz]
+    lib.scd_int4_layout.argtypes = [C.POINTER(Int4Desc), i32, i32, psz, psz, psz, psz]
     lib.scd_int4_quantize.argtypes = [C.POINTER(Int4Desc), i32, i32, C.POINTER(vp), C.c_int64, vp, vp]
     lib.scd_int4_dequantize_paged.argtypes = [C.POINTER(Int4Desc), C.POINTER(BatchDesc), i32, vp, C.POINTER(vp), i32, vp]
     for name in ("scd_int4_layout", "scd_int4_quantize", "scd_int4_dequantize_paged"):
         getattr(lib, name).restype = C.c_int
+    lib.scd_fit_query.argtypes = [C.POINTER(FitDesc), C.c_int64, psz]
+    lib.scd_fit_reuse.argtypes = [C.POINTER(FitDesc), vp, vp, C.c_int64, C.c_int64, vp, vp, vp, vp, vp, vp, vp, sz, pi32, vp]
+    lib.scd_fit_query.restype = C.c_int
+    lib.scd_fit_reuse.restype = C.c_int
     lib.scd_last_launch_count.restype = C.c_int32
     lib.scd_profile_enable.argtypes = [i32]
     lib.scd_profile_enable.restype = C.c_int
@@ -274,8 +284,8 @@ def scd_patch(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequenc
 
 
 def scd_int4_layout(desc: Int4Desc, total_tokens: int, n_tensors: int):
-    """(tensor_stride, scale_offset, zero_offset, total_bytes, payload_bytes); pure host arithmetic."""
-    v = [C.c_size_t(0) for _ in range(5)]
+    """(tensor_stride, meta_offset, total_bytes, payload_bytes); pure host arithmetic."""
+    v = [C.c_size_t(0) for _ in range(4)]
     _check(lib.scd_int4_layout(C.byref(desc), total_tokens, n_tensors, *[C.byref(x) for x in v]))
     return tuple(x.value for x in v)
 
@@ -292,6 +302,23 @@ def scd_int4_dequantize_paged(desc: Int4Desc, batch: BatchDesc, packed: torch.Te
     _check(lib.scd_int4_dequantize_paged(C.byref(desc), C.byref(batch), len(pools), _ptr(packed), _ptr_array(pools),
                                          n_blocks, _stream_ptr(stream)))
     return lib.scd_last_launch_count()
+
+
+def scd_fit_query(desc: FitDesc, n_rows: int) -> int:
+    ws = C.c_size_t(0)
+    _check(lib.scd_fit_query(C.byref(desc), n_rows, C.byref(ws)))
+    return ws.value
+
+
+def scd_fit_reuse(desc: FitDesc, a: torch.Tensor, b: torch.Tensor, n_rows: int, row_stride: int, w_enc: torch.Tensor,
+                  w_dec_a: Optional[torch.Tensor], w_dec_b: torch.Tensor, mu_a: Optional[torch.Tensor],
+                  mu_b: Optional[torch.Tensor], sigma: Optional[torch.Tensor], workspace: torch.Tensor, stream=None) -> int:
+    """Returns the Jacobi sweeps (joint solve, ridge solve).  Synchronises the stream (not a hot call)."""
+    sweeps = (C.c_int32 * 2)()
+    _check(lib.scd_fit_reuse(C.byref(desc), _ptr(a), _ptr(b), n_rows, row_stride, _ptr(w_enc), _ptr(w_dec_a), _ptr(w_dec_b),
+                             _ptr(mu_a), _ptr(mu_b), _ptr(sigma), _ptr(workspace),
+                             workspace.numel() * workspace.element_size(), sweeps, _stream_ptr(stream)))
+    return sweeps[0], sweeps[1]
 
 
 def profile_enable(on: bool) -> None:

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["scd_host.cu", "scd_prep.cu", "scd_simt.cu", "scd_tc.cu", "scd_tc_kv.cu", "scd_int4.cu"]
+SOURCES = ["scd_host.cu", "scd_prep.cu", "scd_simt.cu", "scd_tc.cu", "scd_tc_kv.cu", "scd_int4.cu", "scd_fit.cu"]
 HEADERS = ["scd_internal.h", "scd_device.cuh", "scd_tc.h", "scd_tc_common.cuh", "ptx.cuh", os.path.join(ROOT, "include", "scd.h")]
 LIB = os.path.join(HERE, "libscd.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -31,7 +31,8 @@ enum EpiKind : int {
 // ids under which scd_profile_fetch reports the launches of the tensor-core path
 enum ProfId : int {
   SCD_PROF_ENCODE = 100, SCD_PROF_ENCODE_K = 101, SCD_PROF_REUSE_DECODE = 110, SCD_PROF_PATCH_GEMM1 = 120,
-  SCD_PROF_PATCH_GEMM2 = 130, SCD_PROF_PATCH_GEMM3 = 140, SCD_PROF_INT4_QUANT = 200, SCD_PROF_INT4_DEQUANT = 201
+  SCD_PROF_PATCH_GEMM2 = 130, SCD_PROF_PATCH_GEMM3 = 140, SCD_PROF_INT4_QUANT = 200, SCD_PROF_INT4_DEQUANT = 201,
+  SCD_PROF_FIT_GRAM = 300
 };
 
 enum AMode : int {

@@ -819,6 +819,12 @@ static scd_status_t make_map(CUtensorMap* m, const void* base, uint64_t d0, uint
   return SCD_OK;
 }
 
+// scd_fit.cu: bf16 matrix [rows][cols] (cols contiguous, row pitch in bytes), box {64, box_rows}, 128-B swizzle
+scd_status_t tc_make_map_2d_bf16(CUtensorMap* m, const void* base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,
+                                 uint32_t box_rows) {
+  return make_map(m, base, cols, rows, 1, row_pitch_bytes, row_pitch_bytes * rows, box_rows, 1);
+}
+
 // e4m3 code segments [n_seg][T][r] (1 byte per code): box {64, 128, 1}, no swizzle (expanded in shared memory)
 static scd_status_t make_code_map_u8(CUtensorMap* m, const void* base, uint64_t r, uint64_t T, uint64_t n_seg,
                                      uint64_t seg_stride) {

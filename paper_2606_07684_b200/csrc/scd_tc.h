@@ -21,4 +21,8 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
                       void* ws_act, void* ws_u, float* ws_ss, int group, size_t act_stride, size_t u_stride, size_t ss_stride,
                       const size_t* off, const size_t* soff, cudaStream_t s);
 
+// TMA descriptor of a bf16 matrix [rows][cols] (K-major operand of the tcgen05 kernels): box {64, box_rows}, 128-B swizzle
+scd_status_t tc_make_map_2d_bf16(CUtensorMap* m, const void* base, uint64_t cols, uint64_t rows, uint64_t row_pitch_bytes,
+                                 uint32_t box_rows);
+
 }  // namespace scd

@@ -64,7 +64,8 @@ class CodecProblem:
         if a.kind == W.REUSE:
             return B.reuse_layer_desc(enc_k=a.enc_k, enc_v=a.enc_v, dec_k=a.dec_k, dec_v=a.dec_v,
                                       mean_src_k=mk(a.mean_k), mean_src_v=mk(a.mean_v),
-                                      mean_dst_k=mk(a.mean_k), mean_dst_v=mk(a.mean_v))
+                                      mean_dst_k=mk(a.mean_k if a.mean_dst_k is None else a.mean_dst_k),
+                                      mean_dst_v=mk(a.mean_v if a.mean_dst_v is None else a.mean_dst_v))
         return B.patch_layer_desc(enc_h=a.enc_h, mean_src_h=mk(a.mean_h), w1=a.w1, b1=a.b1, w2=a.w2, b2=a.b2,
                                   norm_gamma=a.gamma, w_k=a.w_k, w_v=a.w_v, b_k=a.b_k, b_v=a.b_v)
 

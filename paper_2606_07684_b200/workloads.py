@@ -202,6 +202,8 @@ class LayerArtifacts:
     dec_v: Optional[torch.Tensor] = None
     mean_k: Optional[torch.Tensor] = None     # [D] fp32 (src = dst)
     mean_v: Optional[torch.Tensor] = None
+    mean_dst_k: Optional[torch.Tensor] = None # [D] fp32 consumer-side mean when it differs from the producer's (fitted pairs)
+    mean_dst_v: Optional[torch.Tensor] = None
     enc_h: Optional[torch.Tensor] = None      # [d, r]
     mean_h: Optional[torch.Tensor] = None     # [d] fp32
     w1: Optional[torch.Tensor] = None         # [r, d_a]

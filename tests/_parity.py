@@ -87,7 +87,9 @@ def oracle_layer(prob, l: int) -> O.Layer:
     mk = (lambda t: np64(t)) if prob.use_means else (lambda t: None)
     if a.kind == W.REUSE:
         return O.Layer(O.REUSE, enc_k=np64(a.enc_k), enc_v=np64(a.enc_v), dec_k=np64(a.dec_k), dec_v=np64(a.dec_v),
-                       mean_src_k=mk(a.mean_k), mean_src_v=mk(a.mean_v), mean_dst_k=mk(a.mean_k), mean_dst_v=mk(a.mean_v))
+                       mean_src_k=mk(a.mean_k), mean_src_v=mk(a.mean_v),
+                       mean_dst_k=mk(a.mean_k if a.mean_dst_k is None else a.mean_dst_k),
+                       mean_dst_v=mk(a.mean_v if a.mean_dst_v is None else a.mean_dst_v))
     return O.Layer(O.PATCH, enc_h=np64(a.enc_h), mean_src_h=mk(a.mean_h), w1=np64(a.w1), b1=np64(a.b1), w2=np64(a.w2),
                    b2=np64(a.b2), norm_gamma=np64(a.gamma), w_k=np64(a.w_k), w_v=np64(a.w_v), b_k=np64(a.b_k),
                    b_v=np64(a.b_v))

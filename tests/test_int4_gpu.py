@@ -29,7 +29,7 @@ def _case(cfg, group, device, n_layers, stride_pad=0, seed=0):
             x[0, 5] = 300.0                                       # an outlier
         src.append(x.to(torch.bfloat16).to(device))
     desc = B.Int4Desc(cfg.n_kv_heads, cfg.head_dim, cfg.block_size, group)
-    stride_b, soff, zoff, total, payload = B.scd_int4_layout(desc, T, len(src))
+    stride_b, moff, total, payload = B.scd_int4_layout(desc, T, len(src))
     assert payload == Q.payload_bytes(T, D, group, len(src))
     packed = torch.full((total + 4096,), 0xA5, dtype=torch.uint8, device=device)
     pools = [torch.full((batch.n_blocks, cfg.block_size, cfg.n_kv_heads, cfg.head_dim), SENTINEL, dtype=torch.int16,
@@ -48,12 +48,12 @@ def _case(cfg, group, device, n_layers, stride_pad=0, seed=0):
         q, want_packed, s, z = Q.quantize(xf, group)
         base = i * stride_b
         got_q = pk[base:base + T * D // 2].reshape(T, D // 2)
-        got_s = torch.from_numpy(pk[base + soff:base + soff + T * (D // group) * 2].copy()).view(torch.bfloat16).float().numpy().reshape(T, -1)
-        got_z = torch.from_numpy(pk[base + zoff:base + zoff + T * (D // group) * 2].copy()).view(torch.bfloat16).float().numpy().reshape(T, -1)
+        meta = torch.from_numpy(pk[base + moff:base + moff + T * (D // group) * 4].copy()).view(torch.bfloat16).float().numpy().reshape(T, -1, 2)
+        got_s, got_z = meta[:, :, 0], meta[:, :, 1]
         np.testing.assert_array_equal(got_q, want_packed)
         np.testing.assert_array_equal(got_s, s)
         np.testing.assert_array_equal(got_z, z)
-        for b0, n in ((base, T * D // 2), (base + soff, T * (D // group) * 2), (base + zoff, T * (D // group) * 2)):
+        for b0, n in ((base, T * D // 2), (base + moff, T * (D // group) * 4)):
             written[b0:b0 + n] = True
         want = Q.dequantize(q, s, z, group)
         pool = pools[i].view(torch.int16).cpu().numpy().reshape(-1, D)

@@ -159,10 +159,10 @@ def test_int4_layout_matches_oracle_payload_and_rejects_bad_groups(B):
     for group in (32, 64, 128):
         desc = B.Int4Desc(8, 128, 16, group)
         for T, n in ((1000, 3), (1, 1), (8192, 64)):
-            stride, soff, zoff, total, payload = B.scd_int4_layout(desc, T, n)
+            stride, moff, total, payload = B.scd_int4_layout(desc, T, n)
             assert payload == Q.payload_bytes(T, 1024, group, n)
-            assert stride % 128 == 0 and soff % 128 == 0 and zoff % 128 == 0 and total == stride * n
-            assert T * 512 <= soff and soff + T * (1024 // group) * 2 <= zoff and zoff + T * (1024 // group) * 2 <= stride
+            assert stride % 128 == 0 and moff % 128 == 0 and total == stride * n
+            assert T * 512 <= moff and moff + T * (1024 // group) * 4 <= stride
     for bad in (B.Int4Desc(8, 128, 16, 16), B.Int4Desc(8, 64, 16, 128), B.Int4Desc(0, 128, 16, 32)):
         with pytest.raises(B.ScdError):
             B.scd_int4_layout(bad, 10, 1)

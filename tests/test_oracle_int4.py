@@ -69,8 +69,9 @@ def _scalar_quant(row, group):
         s = _bf16(_f32(_f32(hi - lo) / 15))
         if s == 0:
             s = Fraction(1)
+        inv = _f32(Fraction(1) / s)
         for x in xs:
-            t = _f32(_f32(x - lo) / s)
+            t = _f32(_f32(x - lo) * inv)
             q.append(max(0, min(15, _rint(t))))
         s_out.append(s)
         z_out.append(lo)
