@@ -127,6 +127,15 @@ typedef struct {
   const void *const *v;
   const void *const *h;              /* [n_layers] -> [total_tokens, d_model]; PATCH layers read   */
   int64_t kv_token_stride, kv_head_stride, h_token_stride;   /* in elements              */
+  /* Paged producer cache ("native cache semantics"): when page_table is not
+   * NULL, k[l] / v[l] point to the PRODUCER's paged pools [n_blocks, block_size, H_kv, d_h] (dense heads;
+   * kv_token_stride = elements between slots) and token t of request b is read from slot
+   * page_table[b][t / bs] * bs + t % bs -- the encode gathers rows through the table (TMA tile::gather4), no
+   * packed copy is made.  h stays packed [total_tokens, d_model].  The table lives on the device and is trusted:
+   * a page id outside [0, n_blocks) reads slot 0 instead (that token's codes are then meaningless, nothing is
+   * read out of bounds).  bf16 states only. */
+  const int32_t *page_table;         /* DEVICE [n_seqs, max_pages_per_seq] or NULL (packed rows) */
+  int32_t max_pages_per_seq, n_blocks;
 } scd_src_t;
 
 /* Consumer paged pool.  k_pool, v_pool are HOST arrays of n_layers DEVICE pointers, each

@@ -166,6 +166,14 @@ def slot_mapping(batch: Batch, block_size: int) -> np.ndarray:
     return slots
 
 
+def read_paged(pool: np.ndarray, slots: np.ndarray) -> np.ndarray:
+    """Packed rows of a batch read back from a paged pool [n_blocks, bs, H_kv, d_h] (or [n_slots, D]): row n of the
+    batch is the pool row at slots[n].  The producer's cache may be paged too ("native cache semantics",
+    PAPER.md:610): encode then reads K_A / V_A through the producer's own page table."""
+    flat = pool.reshape(-1, pool.shape[-2] * pool.shape[-1]) if pool.ndim == 4 else pool
+    return flat[np.asarray(slots, dtype=np.int64)]
+
+
 def write_paged(pool: np.ndarray, slots: np.ndarray, rows: np.ndarray) -> None:
     """Pool element (slot, head, c) lives at ((slot*H_kv)+head)*d_h + c, i.e. the pool
     viewed as [n_blocks*bs, D] takes row `rows[n]` at index slots[n]."""

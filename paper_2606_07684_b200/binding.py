@@ -67,7 +67,8 @@ class BatchDesc(C.Structure):
 
 class SrcDesc(C.Structure):
     _fields_ = [("k", C.POINTER(C.c_void_p)), ("v", C.POINTER(C.c_void_p)), ("h", C.POINTER(C.c_void_p)),
-                ("kv_token_stride", C.c_int64), ("kv_head_stride", C.c_int64), ("h_token_stride", C.c_int64)]
+                ("kv_token_stride", C.c_int64), ("kv_head_stride", C.c_int64), ("h_token_stride", C.c_int64),
+                ("page_table", C.c_void_p), ("max_pages_per_seq", C.c_int32), ("n_blocks", C.c_int32)]
 
 
 class PagedKV(C.Structure):
@@ -247,9 +248,12 @@ def scd_plan(model: ModelDesc, layers: Sequence[LayerDesc], stream=None) -> Plan
 
 def scd_encode(plan: Plan, batch: BatchDesc, k: Sequence[Optional[torch.Tensor]],
                v: Sequence[Optional[torch.Tensor]], h: Sequence[Optional[torch.Tensor]], codes: torch.Tensor,
-               kv_token_stride: int, kv_head_stride: int, h_token_stride: int, stream=None, layers=None) -> int:
-    """`layers` = (begin, end): the layer-streamed variant scd_encode_layers."""
-    src = SrcDesc(_ptr_array(k), _ptr_array(v), _ptr_array(h), kv_token_stride, kv_head_stride, h_token_stride)
+               kv_token_stride: int, kv_head_stride: int, h_token_stride: int, stream=None, layers=None,
+               src_page_table: Optional[torch.Tensor] = None, src_n_blocks: int = 0) -> int:
+    """`layers` = (begin, end): the layer-streamed variant scd_encode_layers.  `src_page_table` [n_seqs, max_pages]
+    int32: k / v are the producer's paged pools and rows are gathered through it."""
+    src = SrcDesc(_ptr_array(k), _ptr_array(v), _ptr_array(h), kv_token_stride, kv_head_stride, h_token_stride,
+                  _ptr(src_page_table), 0 if src_page_table is None else src_page_table.shape[1], src_n_blocks)
     if layers is None:
         _check(lib.scd_encode(plan.handle, C.byref(batch), C.byref(src), _ptr(codes), _stream_ptr(stream)))
     else:

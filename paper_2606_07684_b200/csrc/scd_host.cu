@@ -544,6 +544,13 @@ scd_status_t scd_encode(const scd_plan_t* plan, const scd_batch_t* batch, const 
   if (has_reuse && (src->kv_head_stride < m.head_dim || src->kv_token_stride < (int64_t)m.n_kv_heads * m.head_dim))
     return fail(SCD_E_SHAPE, "kv strides smaller than the tensor");
   if (!plan->patches.empty() && src->h_token_stride < m.d_model) return fail(SCD_E_SHAPE, "h_token_stride < d_model");
+  if (src->page_table && has_reuse) {
+    if (!plan->use_tc) return fail(SCD_E_UNSUPPORTED, "paged producer source: bf16 states only");
+    if (src->kv_head_stride != m.head_dim) return fail(SCD_E_UNSUPPORTED, "paged producer source needs dense heads");
+    if (src->n_blocks < 1 || src->max_pages_per_seq < 1) return fail(SCD_E_ARG, "paged producer source: n_blocks / max_pages_per_seq");
+    if ((int64_t)src->max_pages_per_seq * m.block_size < batch->max_seqlen)
+      return fail(SCD_E_SHAPE, "producer page table too narrow for max_seqlen");
+  }
   for (const SegPlan& sp : plan->segs) {
     if (!layer_in_window(sp.layer)) continue;
     const void* a = sp.branch == SCD_BRANCH_K ? src->k[sp.layer] : sp.branch == SCD_BRANCH_V ? src->v[sp.layer] : src->h[sp.layer];

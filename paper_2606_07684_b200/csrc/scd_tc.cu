@@ -314,6 +314,43 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   if (AMODE != A_PLAIN) ptx::setmaxnreg_dec<24>();
   if (warp == 0) {
     // ============================== TMA producer ==============================
+    if (P.a_gather) {
+      // Paged producer cache: the tile's 128 token rows sit at the slots the producer's page table gives them.  Lane l
+      // owns rows 4l .. 4l+3 and fetches them with one tile::gather4 per k-block (32 gathers = one A tile); lane 0
+      // also arms the barrier and loads the B tile.  Rows beyond M (and page ids outside the pool) read slot 0.
+      int stage = 0;
+      uint32_t phase = 0;
+      int cur_m = -1;
+      int r4[4] = {0, 0, 0, 0};
+      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        int m_tile, n_tile, seg_i;
+        tile_decode(P, tile, m_tile, n_tile, seg_i);
+        const TcSeg& sg = P.segs[seg_i];
+        const CUtensorMap* am = &P.a_maps[sg.a_map];
+        const CUtensorMap* bm = P.b_maps + sg.b_map;
+        if (m_tile != cur_m) {
+          cur_m = m_tile;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int row = m_tile * BLOCK_M + lane * 4 + i;
+            int pos;
+            long long slot = -1;
+            if (row < P.M) row_to_pos_slot(P.batch, row, pos, slot);
+            r4[i] = slot < 0 ? 0 : (int)slot;
+          }
+        }
+        for (int kb = 0; kb < P.num_kb; ++kb) {
+          ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
+          if (lane == 0) {
+            ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES + b_stage_bytes);
+            ptx::tma_load_2d(smem_b + stage * b_stage_bytes, bm, &bars->full[stage], kb * BLOCK_K, n_tile * block_n);
+          }
+          __syncwarp();
+          ptx::tma_gather4_2d(smem_a + stage * A_STAGE_BYTES + lane * 512, am, &bars->full[stage], kb * BLOCK_K, r4[0], r4[1], r4[2], r4[3]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    } else
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
@@ -825,6 +862,22 @@ scd_status_t tc_make_map_2d_bf16(CUtensorMap* m, const void* base, uint64_t cols
   return make_map(m, base, cols, rows, 1, row_pitch_bytes, row_pitch_bytes * rows, box_rows, 1);
 }
 
+// paged producer pool [n_slots][width] (row pitch in bytes): 2-D, box {64, 1} for tile::gather4, 128-B swizzle
+static scd_status_t make_gather_map(CUtensorMap* m, const void* base, uint64_t width, uint64_t n_slots, uint64_t pitch_bytes) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return fail(SCD_E_CUDA, "cuTensorMapEncodeTiled entry point not found");
+  cuuint64_t dims[2] = {width, n_slots};
+  cuuint64_t strides[1] = {pitch_bytes};
+  cuuint32_t box[2] = {BLOCK_K, 1};
+  cuuint32_t es[2] = {1, 1};
+  CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, es,
+                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(SCD_E_CUDA, "cuTensorMapEncodeTiled (gather %llu x %llu) failed (%d)", (unsigned long long)n_slots,
+                                     (unsigned long long)width, (int)r);
+  return SCD_OK;
+}
+
 // e4m3 code segments [n_seg][T][r] (1 byte per code): box {64, 128, 1}, no swizzle (expanded in shared memory)
 static scd_status_t make_code_map_u8(CUtensorMap* m, const void* base, uint64_t r, uint64_t T, uint64_t n_seg,
                                      uint64_t seg_stride) {
@@ -945,7 +998,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n, compact, (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2);
   P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
-  P.a_prefetch = (EPI == EPI_CODES) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
+  P.a_prefetch = (EPI == EPI_CODES && !P.a_gather) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
   P.msb = P.m_tiles;
   if (P.n_tiles > 1) {
     const long long a_tile_bytes = (long long)BLOCK_M * P.K * 2;
@@ -1030,6 +1083,13 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
     P.K = s0.width;
     P.block_n = pick_block_n_cover(s0.rank);
     P.a_kb_per_head = (s0.branch != SCD_BRANCH_H && !dense_kv) ? m.head_dim / BLOCK_K : 0;
+    const bool gather = src->page_table != nullptr && s0.branch != SCD_BRANCH_H;
+    if (gather) {                       // rows of the K / V tiles come through the producer's page table
+      P.a_gather = 1;
+      P.batch.page_table = src->page_table;
+      P.batch.max_pages_per_seq = src->max_pages_per_seq;
+      P.batch.n_blocks = src->n_blocks;
+    }
     for (size_t q = i; q < j; ++q) {
       const SegPlan& sp = p->segs[q];
       const int key = sp.layer * 3 + sp.branch;
@@ -1046,7 +1106,9 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
                       (uint64_t)src->h_token_stride * 2 * T, BLOCK_M, 1);
       else {
         const void* a = sp.branch == SCD_BRANCH_K ? src->k[sp.layer] : src->v[sp.layer];
-        if (dense_kv)
+        if (gather)
+          st = make_gather_map(am, a, p->D, (uint64_t)src->n_blocks * m.block_size, (uint64_t)src->kv_token_stride * 2);
+        else if (dense_kv)
           st = make_map(am, a, p->D, T, 1, (uint64_t)src->kv_token_stride * 2, (uint64_t)src->kv_token_stride * 2 * T,
                         BLOCK_M, 1);
         else

@@ -48,6 +48,7 @@ struct TcParams {
   int32_t prof_id;                    // host only: id under which scd_profile_* reports the launch
   int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
   int32_t a_is_codes;                 // paged-KV kernel: A is a code segment (e4m3 codes are widened in shared memory)
+  int32_t a_gather;                   // generic kernel: A rows are gathered through P.batch.page_table (paged producer cache)
   long long pool_slots;               // paged epilogues: n_blocks * block_size (slot numbers are kept as int32)
 };
 

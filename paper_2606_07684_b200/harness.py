@@ -90,9 +90,10 @@ class CodecProblem:
         return k, v, h
 
     # ---- the three hot calls ---------------------------------------------------------
-    def encode(self, k, v, h, stream=None, layers=None) -> int:
+    def encode(self, k, v, h, stream=None, layers=None, src_page_table=None, src_n_blocks=0) -> int:
         cfg = self.cfg
-        return B.scd_encode(self.plan, self.bdesc, k, v, h, self.codes, cfg.D, cfg.head_dim, cfg.d_model, stream, layers)
+        return B.scd_encode(self.plan, self.bdesc, k, v, h, self.codes, cfg.D, cfg.head_dim, cfg.d_model, stream, layers,
+                            src_page_table, src_n_blocks)
 
     def reuse_decode(self, stream=None, layers=None) -> int:
         return B.scd_reuse_decode(self.plan, self.bdesc, self.codes, self.k_pool, self.v_pool, self.batch.n_blocks, stream,

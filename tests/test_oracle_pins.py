@@ -405,6 +405,14 @@ def test_slot_mapping_bruteforce_and_identity():
     np.testing.assert_array_equal(flat[slots], rows)
     untouched = np.setdiff1d(np.arange(flat.shape[0]), slots)
     assert np.all(flat[untouched] == -7.0)
+    # read_paged (paged producer cache) is the inverse walk: token by token through the table
+    got = O.read_paged(pool, slots)
+    n = 0
+    for i, l in enumerate(lens):
+        for t in range(l):
+            np.testing.assert_array_equal(got[n], pool[table[i][t // bs], t % bs].reshape(-1))
+            n += 1
+    np.testing.assert_array_equal(got, rows)
 
 
 def test_route_and_payload():

@@ -407,3 +407,49 @@ def test_full_size_sampled_parity(name, rank, cuda_device):
     rows = P.sample_rows(prob, FULL_SAMPLE[name])
     res = _run_all(prob, rows=rows, roped=False)
     print(name, rank, res)
+
+
+@pytest.mark.parametrize("name", ["llama3_8b_ragged", "mistral_7b_32k_fp8"])
+def test_paged_producer_source(name, cuda_device):
+    """the producer's K / V live in ITS paged cache (own page table, own permutation, junk in
+    the unused slots) and scd_encode gathers them through that table (TMA tile::gather4).  The codes must equal,
+    bit for bit, those of the same rows handed over packed, and match the oracle reading the pool through
+    O.read_paged."""
+    cfg = MINI[name].scaled(ragged_range=(5, 1, 400), permute_pages=True) if name == "llama3_8b_ragged" else MINI[name]
+    prob = _problem(cfg, cuda_device)
+    k, v, h = prob.make_sources()
+    k = P.roped_producer_k(prob, k)
+    prob.encode(k, v, h)
+    torch.cuda.synchronize()
+    want = prob.codes.clone()
+    # the producer's own paging: a different permutation over a larger pool
+    bs, T = cfg.block_size, prob.T
+    g = torch.Generator().manual_seed(99)
+    pages = [(l + bs - 1) // bs for l in prob.batch.seqlens]
+    n_blocks = sum(pages) + 7
+    ids = torch.randperm(n_blocks, generator=g)
+    table = torch.full((len(pages), max(pages) + 2), -1, dtype=torch.int32)
+    at = 0
+    for i, n in enumerate(pages):
+        table[i, :n] = ids[at:at + n].to(torch.int32)
+        at += n
+    ob = O.Batch(prob.batch.cu_seqlens.cpu().numpy().astype(np.int64), table.numpy().astype(np.int64), None)
+    slots = torch.from_numpy(O.slot_mapping(ob, bs)).to(cuda_device)
+    kp, vp = [None] * cfg.n_layers, [None] * cfg.n_layers
+    for l in range(cfg.n_layers):
+        if k[l] is None:
+            continue
+        for src, dst in ((k, kp), (v, vp)):
+            pool = torch.randn(n_blocks * bs, cfg.D, generator=g).to(torch.bfloat16).to(cuda_device)
+            pool[slots] = src[l].reshape(T, cfg.D)
+            dst[l] = pool
+            # the oracle's reading of the pool gives back the packed rows
+            np.testing.assert_array_equal(O.read_paged(pool.float().cpu().numpy(), slots.cpu().numpy()),
+                                          src[l].reshape(T, cfg.D).float().cpu().numpy())
+    prob.codes.fill_(0xA5)
+    prob.encode(kp, vp, h, src_page_table=table.to(cuda_device), src_n_blocks=n_blocks)
+    torch.cuda.synchronize()
+    for b, e in prob.code_ranges():
+        assert torch.equal(prob.codes[b:e], want[b:e]), "codes gathered through the producer's page table differ"
+    assert prob.guard_violations() == (0, 0)
+    P.check_encode(prob, k, v, h)
