@@ -139,11 +139,19 @@ typedef struct {
 } scd_src_t;
 
 /* Consumer paged pool.  k_pool, v_pool are HOST arrays of n_layers DEVICE pointers, each
- * -> [n_blocks, block_size, H_kv, d_h] in state_dtype. */
+ * -> [n_blocks, block_size, H_kv, d_h] in state_dtype.
+ * fp8 pools (build extension, DESIGN.md section 2 U20): pool_e4m3 != 0 makes the pools
+ * [n_blocks, block_size, H_kv, d_h] e4m3fn BYTES with one fp32 scale per (slot, head) in k_scale[l] / v_scale[l]
+ * -> [n_blocks, block_size, H_kv]: for each head of a token, x = the bf16 value the codec would have stored,
+ * s = amax_head / 448 (1 if the head is all zero), stored byte = e4m3_rne_sat(x * (1 / s)) in IEEE fp32.
+ * bf16 states, head_dim 128, HALF RoPE only (else SCD_E_UNSUPPORTED). */
 typedef struct {
   void *const *k_pool;
   void *const *v_pool;
   int32_t n_blocks;
+  int32_t pool_e4m3;                 /* 0: pools in state_dtype; 1: e4m3 bytes + per-(slot, head) fp32 scales */
+  float *const *k_scale;             /* HOST arrays of n_layers DEVICE pointers, used when pool_e4m3 != 0 */
+  float *const *v_scale;
 } scd_paged_kv_t;
 
 /* Create a plan: validates, classifies layers (REUSE | PATCH), copies and repacks the

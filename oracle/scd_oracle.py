@@ -280,6 +280,27 @@ def pack_codes(z: np.ndarray, code_dtype: int) -> Tuple[np.ndarray, Optional[np.
     return q, s
 
 
+def quantize_pool(y: np.ndarray, n_heads: int) -> Tuple[np.ndarray, np.ndarray]:
+    """fp8 K/V pools (build extension, DESIGN.md section 2 U20).  y [T, D] = the K or V rows the
+    consumer stores (fp64).  Per (token, head): x = bf16(y) (the value a bf16 pool would hold), s = amax / 448 in fp32
+    (1 for an all-zero head), byte = e4m3_rne_sat(x * (1 / s)) with 1 / s and the product rounded to fp32 -- the
+    decision is taken in the kernel's precision.  Returns (bytes [T, D] uint8, scales [T, n_heads] fp32)."""
+    T, D = y.shape
+    x = round_to_bf16(y).astype(np.float32).reshape(T, n_heads, D // n_heads)
+    amax = np.max(np.abs(x), axis=2)
+    s = np.where(amax > 0, (amax / np.float32(E4M3_MAX)).astype(np.float32), np.float32(1.0)).astype(np.float32)
+    inv = (np.float32(1.0) / s).astype(np.float32)
+    t = (x * inv[:, :, None]).astype(np.float32)
+    return e4m3_quantize(t.astype(np.float64)).reshape(T, D), s
+
+
+def dequantize_pool(q: np.ndarray, s: np.ndarray) -> np.ndarray:
+    """bytes [T, D], scales [T, H] -> fp64 values (exact): s * value(byte)."""
+    T, D = q.shape
+    H = s.shape[1]
+    return (E4M3_VALUES[q].reshape(T, H, D // H) * s.astype(np.float64)[:, :, None]).reshape(T, D)
+
+
 def unpack_codes(q: np.ndarray, scale: Optional[np.ndarray], code_dtype: int) -> np.ndarray:
     """Stored codes -> fp64 (exact).  e4m3: s * value(q)."""
     if code_dtype == E4M3_ROWSCALE:

@@ -72,7 +72,8 @@ class SrcDesc(C.Structure):
 
 
 class PagedKV(C.Structure):
-    _fields_ = [("k_pool", C.POINTER(C.c_void_p)), ("v_pool", C.POINTER(C.c_void_p)), ("n_blocks", C.c_int32)]
+    _fields_ = [("k_pool", C.POINTER(C.c_void_p)), ("v_pool", C.POINTER(C.c_void_p)), ("n_blocks", C.c_int32),
+                ("pool_e4m3", C.c_int32), ("k_scale", C.POINTER(C.c_void_p)), ("v_scale", C.POINTER(C.c_void_p))]
 
 
 class Int4Desc(C.Structure):
@@ -262,9 +263,17 @@ def scd_encode(plan: Plan, batch: BatchDesc, k: Sequence[Optional[torch.Tensor]]
     return lib.scd_last_launch_count()
 
 
+def _paged_kv(k_pool, v_pool, n_blocks, k_scale, v_scale) -> PagedKV:
+    if k_scale is None:
+        return PagedKV(_ptr_array(k_pool), _ptr_array(v_pool), n_blocks, 0, None, None)
+    return PagedKV(_ptr_array(k_pool), _ptr_array(v_pool), n_blocks, 1, _ptr_array(k_scale), _ptr_array(v_scale))
+
+
 def scd_reuse_decode(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequence[Optional[torch.Tensor]],
-                     v_pool: Sequence[Optional[torch.Tensor]], n_blocks: int, stream=None, layers=None) -> int:
-    kv = PagedKV(_ptr_array(k_pool), _ptr_array(v_pool), n_blocks)
+                     v_pool: Sequence[Optional[torch.Tensor]], n_blocks: int, stream=None, layers=None,
+                     k_scale=None, v_scale=None) -> int:
+    """k_scale / v_scale (lists of fp32 tensors [n_blocks, bs, H_kv]): the pools are e4m3 bytes (fp8 pools)."""
+    kv = _paged_kv(k_pool, v_pool, n_blocks, k_scale, v_scale)
     if layers is None:
         _check(lib.scd_reuse_decode(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _stream_ptr(stream)))
     else:
@@ -275,8 +284,8 @@ def scd_reuse_decode(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: 
 
 def scd_patch(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequence[Optional[torch.Tensor]],
               v_pool: Sequence[Optional[torch.Tensor]], n_blocks: int, workspace: Optional[torch.Tensor],
-              stream=None, layers=None) -> int:
-    kv = PagedKV(_ptr_array(k_pool), _ptr_array(v_pool), n_blocks)
+              stream=None, layers=None, k_scale=None, v_scale=None) -> int:
+    kv = _paged_kv(k_pool, v_pool, n_blocks, k_scale, v_scale)
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     if layers is None:
         _check(lib.scd_patch(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _ptr(workspace), ws_bytes,

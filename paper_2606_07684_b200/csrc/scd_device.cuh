@@ -22,6 +22,10 @@ template <> __device__ __forceinline__ __nv_bfloat16 from_float<__nv_bfloat16>(f
 __device__ __forceinline__ uint8_t float_to_e4m3_sat(float v) {
   return (uint8_t)__nv_cvt_float_to_fp8(v, __NV_SATFINITE, __NV_E4M3);
 }
+// two values at once: one cvt.rn.satfinite.e4m3x2.f32 (low byte = a)
+__device__ __forceinline__ uint32_t float2_to_e4m3x2_sat(float a, float b) {
+  return (uint32_t)__nv_cvt_float2_to_fp8x2(make_float2(a, b), __NV_SATFINITE, __NV_E4M3);
+}
 __device__ __forceinline__ float e4m3_to_float(uint8_t b) {
   __half_raw h = __nv_cvt_fp8_to_halfraw((__nv_fp8_storage_t)b, __NV_E4M3);
   return __half2float(__half(h));

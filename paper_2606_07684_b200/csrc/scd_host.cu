@@ -598,6 +598,13 @@ static scd_status_t check_pools(const scd_plan_t* plan, const scd_paged_kv_t* kv
     if (!kv->k_pool[l] || !kv->v_pool[l]) return fail(SCD_E_ARG, "pool of layer %d is NULL", l);
     if (!aligned(kv->k_pool[l], 16) || !aligned(kv->v_pool[l], 16))
       return fail(SCD_E_ALIGN, "pool of layer %d not 16-byte aligned", l);
+    if (kv->pool_e4m3 && (!kv->k_scale || !kv->v_scale || !kv->k_scale[l] || !kv->v_scale[l]))
+      return fail(SCD_E_ARG, "fp8 pools: scale array of layer %d is NULL", l);
+  }
+  if (kv->pool_e4m3) {
+    const scd_model_desc_t& m = plan->model;
+    if (!plan->use_tc || m.head_dim != 128 || m.rope_style != SCD_ROPE_HALF)
+      return fail(SCD_E_UNSUPPORTED, "fp8 pools need bf16 states, head_dim 128 and HALF RoPE");
   }
   return SCD_OK;
 }

@@ -664,11 +664,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
                 uint32_t w[4];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                  uint32_t b = 0;
-#pragma unroll
-                  for (int y = 0; y < 4; ++y)
-                    b |= (uint32_t)float_to_e4m3_sat(__fdiv_rn(v[q * 16 + e * 4 + y], e4_scale)) << (8 * y);
-                  w[e] = b;
+                  w[e] = float2_to_e4m3x2_sat(__fdiv_rn(v[q * 16 + e * 4], e4_scale), __fdiv_rn(v[q * 16 + e * 4 + 1], e4_scale)) |
+                         (float2_to_e4m3x2_sat(__fdiv_rn(v[q * 16 + e * 4 + 2], e4_scale), __fdiv_rn(v[q * 16 + e * 4 + 3], e4_scale)) << 16);
                 }
                 stg_put(stg, pitch, lane, ((c - c0) >> 4) + q, make_uint4(w[0], w[1], w[2], w[3]));
               }
@@ -1177,6 +1174,7 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
       TcSeg& sg = P.segs[q - i];
       sg.col_vec = sp.mean_dst;
       sg.out0 = sp.branch == SCD_BRANCH_K ? kv->k_pool[sp.layer] : kv->v_pool[sp.layer];
+      if (kv->pool_e4m3) sg.scale0 = sp.branch == SCD_BRANCH_K ? kv->k_scale[sp.layer] : kv->v_scale[sp.layer];
       sg.rope_cols = (sp.branch == SCD_BRANCH_K && m.rope_on_reuse_k) ? p->D : 0;
       sg.b_map = nseg_all + sp.seg_index;
       sg.a_scale = e4 ? (const float*)((const char*)codes + soff[key]) : nullptr;
@@ -1195,6 +1193,8 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
     P.prof_id = SCD_PROF_REUSE_DECODE;
     P.head_rank = m.reuse_per_head ? s0.rank / m.n_kv_heads : 0;
     P.a_is_codes = 1;
+    P.pool_e4m3 = kv->pool_e4m3 ? 1 : 0;
+    if (P.pool_e4m3 && !tc_kv_eligible(p, P)) return fail(SCD_E_UNSUPPORTED, "fp8 pools: D must be a multiple of 256");
     // the paged-KV kernel takes 256-column tiles of 128-wide heads (e4m3 codes: widened in shared memory by its own
     // warps); anything else runs on the generic kernel
     if (tc_kv_eligible(p, P)) st = launch_tc_kv(p, P, s);
@@ -1275,6 +1275,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
         return st;
       TcSeg& sg = P.segs[q];
       sg.a_map = q; sg.col_vec = pp.bkv; sg.out0 = kv->k_pool[pp.layer]; sg.out1 = kv->v_pool[pp.layer];
+      if (kv->pool_e4m3) { sg.scale0 = kv->k_scale[pp.layer]; sg.scale1 = kv->v_scale[pp.layer]; }
       sg.rowscale_in = rms ? (const float*)((const char*)ws_ss + q * ss_stride) : nullptr;
       sg.rope_cols = D;
       sg.b_map = 2 * nseg + 3 * (int)(j0 + q) + 2;
@@ -1282,7 +1283,9 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     P.prof_id = SCD_PROF_PATCH_GEMM3;
     // long K (d_model >= 1024): the generic kernel with the compact epilogue runs four pipeline stages where the
     // paged-KV kernel has room for three; short K: the paged-KV kernel's faster epilogue wins
-    const bool long_k = G3_GENERIC && d >= 16 * BLOCK_K;
+    P.pool_e4m3 = kv->pool_e4m3 ? 1 : 0;
+    if (P.pool_e4m3 && !tc_kv_eligible(p, P)) return fail(SCD_E_UNSUPPORTED, "fp8 pools: D must be a multiple of 256");
+    const bool long_k = G3_GENERIC && d >= 16 * BLOCK_K && !P.pool_e4m3;   // fp8 pools: only the paged-KV kernel quantises
     if ((st = (!long_k && tc_kv_eligible(p, P)) ? launch_tc_kv(p, P, s)
                                                                                        : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK)
       return st;

@@ -21,6 +21,8 @@ struct TcSeg {
   void* out0;
   void* out1;
   float* aux;
+  float* scale0;             // fp8 pools: per-(slot, head) scales of out0 / out1
+  float* scale1;
   const float* rowscale_in;  // NORM_RMS: sum-of-squares partials [n_partials][M]
   int32_t a_map, a_z, b_map, rope_cols;
 };
@@ -48,6 +50,7 @@ struct TcParams {
   int32_t prof_id;                    // host only: id under which scd_profile_* reports the launch
   int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
   int32_t a_is_codes;                 // paged-KV kernel: A is a code segment (e4m3 codes are widened in shared memory)
+  int32_t pool_e4m3;                  // paged-KV kernel: pools are e4m3 bytes + per-(slot, head) fp32 scales
   int32_t a_gather;                   // generic kernel: A rows are gathered through P.batch.page_table (paged producer cache)
   long long pool_slots;               // paged epilogues: n_blocks * block_size (slot numbers are kept as int32)
 };

@@ -128,9 +128,13 @@ constexpr int KV_NTHREADS_E4 = KV_NTHREADS + KV_XF_WARPS * 32;          // 768
 // so the raw tile [128 rows x 64 B] lands in the upper half of the A stage and four extra warps (24 in all; registers
 // re-dealt 24 / 104 / 40) widen it in place to the swizzled bf16 tile before the MMA may read it -- exactly (all 254
 // finite codes, test_e4m3_operand_expansion_is_exact_for_every_code); the row scale is applied in the epilogue.
-template <bool DYN, bool SCALED, bool AE4>
+// P8: the pools are e4m3 bytes with one fp32 scale per (slot, head) (fp8 pools, scd.h): the copy-out, which holds a
+// complete bf16 row segment of two heads per warp pass, takes the head's amax over its 16 lanes, and stores 8 bytes per
+// lane plus the scale.
+template <bool DYN, bool SCALED, bool AE4, bool P8>
 __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
   static_assert(!AE4 || (SCALED && !DYN), "e4m3 codes carry row scales; static split");
+  static_assert(!P8 || SCALED, "fp8 pools are built on the scaled variants only");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
@@ -339,7 +343,7 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
     // slot of the row it stores with one broadcast LDS instead of shuffling a 64-bit address out of the owning lane
     const uint32_t wslot = ptx::smem_u32(smem_slot) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 128;
     const uint32_t bar_id = 1 + q;
-    const uint32_t row_stride = (uint32_t)P.pool_width * 2u;  // bytes per slot
+    const uint32_t row_stride = (uint32_t)P.pool_width * (P8 ? 1u : 2u);  // bytes per slot
     // this lane's float4 of the warp's mean / bias slice: tile column for K tiles (runs a | b of both heads) / V tiles
     const int vcol_k = ((lane >> 3) & 1) * 128 + ((lane >> 2) & 1) * 64 + 16 * g + (lane & 3) * 4;
     const int vcol_v = 64 * g + lane * 4;
@@ -428,7 +432,12 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
       const bool to1 = n0 >= P.split;
       // address of this lane's 16 bytes in slot 0 of the tile's pool columns; a row adds slot * row_stride
       const unsigned long long tile_base = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
-                                           (unsigned long long)(to1 ? n0 - P.split : n0) * 2ull + (unsigned long long)lane * 16ull;
+                                           (unsigned long long)(to1 ? n0 - P.split : n0) * (P8 ? 1ull : 2ull) +
+                                           (unsigned long long)lane * (P8 ? 8ull : 16ull);
+      // fp8 pools: scale of this lane's head = [slot][head]
+      float* scale_base = nullptr;
+      if (P8) scale_base = (to1 ? sg.scale1 : sg.scale0) + ((to1 ? n0 - P.split : n0) >> 7) + (lane >> 4);
+      const uint32_t scale_stride = (uint32_t)(P.pool_width >> 7);
 
       // this warp's slice of the tile's mean / bias: wvec[16 * run + i]
       __syncwarp();
@@ -521,9 +530,36 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
           asm volatile("ld.shared.b32 %0, [%1];" : "=r"(sl[i]) : "r"(wslot + r * 4) : "memory");
           v[i] = ptx::lds128(qstg_addr(stg, r, lane));
         }
+        if (P8) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const uint32_t w[4] = {v[i].x, v[i].y, v[i].z, v[i].w};
+            float f[8];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { f[2 * j] = __uint_as_float(w[j] << 16); f[2 * j + 1] = __uint_as_float(w[j] & 0xffff0000u); }
+            float amax = 0.0f;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) amax = fmaxf(amax, fabsf(f[j]));
+#pragma unroll
+            for (int o = 1; o < 16; o <<= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));   // the head's 16 lanes
+            const float sc = amax > 0.0f ? __fdiv_rn(amax, 448.0f) : 1.0f;
+            const float inv = __fdiv_rn(1.0f, sc);
+            uint32_t b0 = 0, b1 = 0;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+              b0 |= float2_to_e4m3x2_sat(__fmul_rn(f[2 * j], inv), __fmul_rn(f[2 * j + 1], inv)) << (16 * j);
+              b1 |= float2_to_e4m3x2_sat(__fmul_rn(f[4 + 2 * j], inv), __fmul_rn(f[5 + 2 * j], inv)) << (16 * j);
+            }
+            if (sl[i] >= 0) {
+              asm volatile("st.global.cs.v2.b32 [%0], {%1, %2};" ::"l"(tile_base + (unsigned long long)(uint32_t)sl[i] * row_stride), "r"(b0), "r"(b1) : "memory");
+              if ((lane & 15) == 0) scale_base[(size_t)(uint32_t)sl[i] * scale_stride] = sc;
+            }
+          }
+        } else {
 #pragma unroll
         for (int i = 0; i < 8; ++i)
           if (sl[i] >= 0) ptx::stg128_cs(tile_base + (unsigned long long)(uint32_t)sl[i] * row_stride, v[i]);
+        }
       }
       cur = nxt;
       tc = tn;
@@ -559,10 +595,13 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   const size_t smem = kv_smem_bytes(P.stages);
   static std::atomic<size_t> configured[SCD_MAX_DEVICES];      // the attribute belongs to (function, device)
   if (configured[p->device].load(std::memory_order_relaxed) < smem) {
-    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false, false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true, true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
     configured[p->device].store(smem, std::memory_order_relaxed);
   }
@@ -579,19 +618,26 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   const bool ae4 = P.code_dtype == SCD_E4M3_ROWSCALE && P.a_is_codes;
   if (ae4 && dyn) return fail(SCD_E_UNSUPPORTED, "internal: e4m3 codes on the dynamically scheduled paged-KV kernel");
   prof_begin(s);
-  if (ae4) {
-    launch_pdl(tc_kv_kernel<false, true, true>, grid, KV_NTHREADS_E4, smem, s, 1, P);
-  } else if (dyn) {
+  const bool p8 = P.pool_e4m3 != 0;
+  if (dyn) {
     P.chunk_tiles = 1;
     P.static_tiles = (int)((long long)total * KV_STATIC_PCT / 100 / grid);
     P.dyn_begin = grid * P.static_tiles;
     P.n_chunks = total - P.dyn_begin;
     P.sched = p->kv_sched + 2 * (p->kv_sched_next.fetch_add(1) % KV_SCHED_SETS);
-    launch_pdl(tc_kv_kernel<true, true, false>, grid, KV_NTHREADS, smem, s, 1, P);
+  }
+  if (ae4) {
+    if (p8) launch_pdl(tc_kv_kernel<false, true, true, true>, grid, KV_NTHREADS_E4, smem, s, 1, P);
+    else launch_pdl(tc_kv_kernel<false, true, true, false>, grid, KV_NTHREADS_E4, smem, s, 1, P);
+  } else if (dyn) {
+    if (p8) launch_pdl(tc_kv_kernel<true, true, false, true>, grid, KV_NTHREADS, smem, s, 1, P);
+    else launch_pdl(tc_kv_kernel<true, true, false, false>, grid, KV_NTHREADS, smem, s, 1, P);
+  } else if (p8) {
+    launch_pdl(tc_kv_kernel<false, true, false, true>, grid, KV_NTHREADS, smem, s, 1, P);
   } else if (scaled) {
-    launch_pdl(tc_kv_kernel<false, true, false>, grid, KV_NTHREADS, smem, s, 1, P);
+    launch_pdl(tc_kv_kernel<false, true, false, false>, grid, KV_NTHREADS, smem, s, 1, P);
   } else {
-    launch_pdl(tc_kv_kernel<false, false, false>, grid, KV_NTHREADS, smem, s, 1, P);
+    launch_pdl(tc_kv_kernel<false, false, false, false>, grid, KV_NTHREADS, smem, s, 1, P);
   }
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();

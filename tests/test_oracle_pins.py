@@ -558,3 +558,34 @@ def test_per_head_mode_against_block_diagonal_and_scalar_loops():
                 assert abs(v1[t, h * d_h + j] - (sum(zv[t, h * r_v + i] * dv[i, j] for i in range(r_v)) + nv[j])) < 1e-12
     # payload: H * r codes per token and branch
     assert O.payload_bytes(ph, [lay_h], 10) == 10 * H * (r_k + r_v) * 4
+
+
+# ------------------------------------------------------------------ fp8 pools (build extension U20)
+def test_quantize_pool_scalar_walk_and_properties():
+    """Per (token, head) walk with torch's fp32 / bf16 / float8 arithmetic as the independent side; the amax element of
+    every head maps to +-448; |deq - x| <= 2^-4 |x| in the normal range; an all-zero head has scale 1 and bytes 0."""
+    H, d_h, T = 3, 16, 9
+    y = rng.standard_normal((T, H * d_h)) * np.array([0.01, 1.0, 30.0]).repeat(d_h)[None, :]
+    y[4, d_h:2 * d_h] = 0.0
+    q, s = O.quantize_pool(y, H)
+    assert q.dtype == np.uint8 and s.dtype == np.float32 and q.shape == y.shape and s.shape == (T, H)
+    xb = torch.from_numpy(y).to(torch.bfloat16).float()
+    for t in range(T):
+        for h in range(H):
+            xs = xb[t, h * d_h:(h + 1) * d_h]
+            amax = xs.abs().max()
+            sc = (amax / torch.tensor(448.0)) if amax > 0 else torch.tensor(1.0)
+            assert float(sc) == float(s[t, h])
+            inv = torch.tensor(1.0) / sc
+            for i in range(d_h):
+                v = float(xs[i] * inv)                       # fp32 product
+                want = torch.tensor(max(-448.0, min(448.0, v))).to(torch.float8_e4m3fn).view(torch.uint8).item()
+                got = int(q[t, h * d_h + i])
+                assert got == want or (O.E4M3_VALUES[got] == 0 and O.E4M3_VALUES[want] == 0), (t, h, i, v, got, want)
+            if amax > 0:
+                assert 448.0 in np.abs(O.E4M3_VALUES[q[t, h * d_h:(h + 1) * d_h]])
+    assert s[4, 1] == 1.0 and not (q[4, d_h:2 * d_h] & 0x7F).any()
+    deq = O.dequantize_pool(q, s)
+    x64 = xb.double().numpy()
+    big = np.abs(x64) >= np.repeat(s, d_h, axis=1) * 2.0 ** -6       # normal range of the head's scale
+    assert np.all(np.abs(deq - x64)[big] <= 2.0 ** -4 * np.abs(x64)[big] * (1 + 1e-6))
