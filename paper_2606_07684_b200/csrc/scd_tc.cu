@@ -54,13 +54,14 @@ static int tc_stg_warp_bytes(int epi, int block_n, bool compact, int out_eb) {
   const int sub = cols < tc_sub_n(epi, false) ? cols : tc_sub_n(epi, false);
   return 32 * ((sub * out_eb + 127) & ~127);       // out_eb: 1 for e4m3 codes, else 2
 }
-static size_t tc_smem_bytes(int block_n, int stages, int stg_warp_bytes, int vec_warp_bytes) {
-  return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2) +
+// b_rows: rows of the B tile a CTA holds per stage (block_n, or half of it when a CTA pair shares the tile)
+static size_t tc_smem_bytes(int b_rows, int stages, int stg_warp_bytes, int vec_warp_bytes) {
+  return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)b_rows * BLOCK_K * 2) +
          EPI_WARPS * (stg_warp_bytes + vec_warp_bytes) + sizeof(TcBarriers);
 }
-static int tc_pick_stages(int block_n, int num_kb, int stg_warp_bytes, int vec_warp_bytes) {
+static int tc_pick_stages(int b_rows, int num_kb, int stg_warp_bytes, int vec_warp_bytes) {
   const size_t budget = 232448 - 1024 - EPI_WARPS * (stg_warp_bytes + vec_warp_bytes) - sizeof(TcBarriers);
-  int st = (int)(budget / (A_STAGE_BYTES + (size_t)block_n * BLOCK_K * 2));
+  int st = (int)(budget / (A_STAGE_BYTES + (size_t)b_rows * BLOCK_K * 2));
   st = st > MAX_STAGES ? MAX_STAGES : st;
   if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty
   return st < 2 ? 2 : st;          // odd rings are fine for deRoPE: a k-block pair may straddle the wrap
@@ -71,19 +72,21 @@ static int tc_pick_stages(int block_n, int num_kb, int stg_warp_bytes, int vec_w
 // n-tile 0, then n-tile 1, ...  The A rows of a super-block (msb x 128 tokens) stay L2-resident while every
 // B slice passes once per super-block, instead of A being re-streamed from HBM once per n-tile when
 // T x K x 2 B outgrows the L2 (PATCH GEMM-2 at 32k tokens: 268-537 MB).  msb >= m_tiles: plain m-fastest order.
-__device__ __forceinline__ void tile_decode(const TcParams& P, int tile, int& m_tile, int& n_tile, int& seg) {
-  const int per_seg = P.m_tiles * P.n_tiles;
+// `mt` = m-tiles of the walk: P.m_tiles, or the number of 256-row pair tiles when CTA pairs share an MMA (P.msb is then
+// in pair tiles too).
+__device__ __forceinline__ void tile_decode(const TcParams& P, int mt, int tile, int& m_tile, int& n_tile, int& seg) {
+  const int per_seg = mt * P.n_tiles;
   seg = tile / per_seg;
   const int t = tile - seg * per_seg;
-  if (P.msb >= P.m_tiles) {
-    n_tile = t / P.m_tiles;
-    m_tile = t - n_tile * P.m_tiles;
+  if (P.msb >= mt) {
+    n_tile = t / mt;
+    m_tile = t - n_tile * mt;
     return;
   }
   const int per_sb = P.msb * P.n_tiles;
   const int sb = t / per_sb;
   const int rem = t - sb * per_sb;
-  const int rows = min(P.msb, P.m_tiles - sb * P.msb);     // the last super-block may be short
+  const int rows = min(P.msb, mt - sb * P.msb);     // the last super-block may be short
   n_tile = rem / rows;
   m_tile = sb * P.msb + (rem - n_tile * rows);
 }
@@ -266,13 +269,23 @@ __device__ __forceinline__ void rope_tile_h128_copy_out(uint32_t stg, unsigned l
 // ---------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------
-template <int EPI, int AMODE>
+// PAIR: two CTAs on the SMs of one TPC (cluster of 2) run ONE tcgen05.mma.cta_group::2 of M = 256: each CTA loads its own
+// 128 rows of A and HALF of the B tile, so a B tile leaves L2 once per 256 output rows and a stage costs 32 KB instead of
+// 48 KB (two more pipeline stages).  The even CTA ("leader") issues the MMAs; loads of both CTAs report to its `full`
+// barriers, its commits are multicast to both CTAs' `empty` / `tmem_full` barriers, and the epilogue warps of both CTAs
+// hand accumulators back on its `tmem_empty` barriers.  Tile = (segment, n-tile, pair of m-tiles).
+template <int EPI, int AMODE, bool PAIR = false>
 __global__ void __launch_bounds__(AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, 1)
 tc_gemm_kernel(const __grid_constant__ TcParams P) {
+  static_assert(!PAIR || AMODE == A_PLAIN, "CTA pairs: plain A operands only");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int block_n = P.block_n;
-  const uint32_t b_stage_bytes = (uint32_t)block_n * BLOCK_K * 2;
+  const uint32_t b_stage_bytes = (uint32_t)block_n * BLOCK_K * (PAIR ? 1 : 2);   // PAIR: this CTA's half of the B tile
+  const uint32_t cta_rank = PAIR ? ptx::cluster_ctarank() : 0u;
+  const int walk_mt = PAIR ? (P.m_tiles + 1) / 2 : P.m_tiles;
+  const int walker = PAIR ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;            // index of this CTA (pair) in the tile walk
+  const int walk_stride = PAIR ? (int)(gridDim.x >> 1) : (int)gridDim.x;
   const int STAGES = P.stages;
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
@@ -283,7 +296,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   TcBarriers* bars = (TcBarriers*)(smem_vec + (vec_smem ? EPI_WARPS * VEC_WARP_BYTES : 0));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int total_tiles = P.n_segs * P.n_tiles * P.m_tiles;
+  const int total_tiles = P.n_segs * P.n_tiles * walk_mt;
 
   if (warp == 0 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
@@ -293,16 +306,22 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
-      ptx::mbar_init(&bars->tmem_empty[a], EPI_WARPS);
+      ptx::mbar_init(&bars->tmem_empty[a], PAIR ? 2 * EPI_WARPS : EPI_WARPS);
     }
     ptx::fence_barrier_init();
   }
   if (warp == 2) {
-    ptx::tmem_alloc<TMEM_COLS>(&bars->tmem_base);
-    ptx::tmem_relinquish();
+    if (PAIR) {
+      ptx::tmem_alloc_cg2<TMEM_COLS>(&bars->tmem_base);
+      ptx::tmem_relinquish_cg2();
+    } else {
+      ptx::tmem_alloc<TMEM_COLS>(&bars->tmem_base);
+      ptx::tmem_relinquish();
+    }
   }
   ptx::tc_fence_before();
-  __syncthreads();
+  if (PAIR) ptx::cluster_sync();        // the peer's barriers exist before anything is sent to them
+  else __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
   ptx::grid_dep_wait();                 // the previous kernel of the stream has completed and flushed
@@ -324,7 +343,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       int r4[4] = {0, 0, 0, 0};
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
         int m_tile, n_tile, seg_i;
-        tile_decode(P, tile, m_tile, n_tile, seg_i);
+        tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
         const TcSeg& sg = P.segs[seg_i];
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
@@ -351,12 +370,35 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         }
       }
     } else
+    if (PAIR) {
+      if (lane == 0) {
+        int stage = 0;
+        uint32_t phase = 0;
+        for (int tile = walker; tile < total_tiles; tile += walk_stride) {
+          int mp, n_tile, seg_i;
+          tile_decode(P, walk_mt, tile, mp, n_tile, seg_i);
+          const int m_tile = 2 * mp + (int)cta_rank;
+          const TcSeg& sg = P.segs[seg_i];
+          const CUtensorMap* am = &P.a_maps[sg.a_map];
+          const CUtensorMap* bm = P.b_maps + sg.b_map;
+          for (int kb = 0; kb < P.num_kb; ++kb) {
+            ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
+            const uint32_t lead_full = ptx::mapa(ptx::smem_u32(&bars->full[stage]), 0);
+            if (cta_rank == 0) ptx::mbar_expect_tx(&bars->full[stage], 2 * (A_STAGE_BYTES + b_stage_bytes));
+            ptx::tma_load_3d_cg2(smem_a + stage * A_STAGE_BYTES, am, lead_full, kb * BLOCK_K, m_tile * BLOCK_M, sg.a_z);
+            ptx::tma_load_2d_cg2(smem_b + stage * b_stage_bytes, bm, lead_full, kb * BLOCK_K,
+                                 n_tile * block_n + (int)cta_rank * (block_n / 2));
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+        }
+      }
+    } else
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
         int m_tile, n_tile, seg_i;
-        tile_decode(P, tile, m_tile, n_tile, seg_i);
+        tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
         const TcSeg& sg = P.segs[seg_i];
         const CUtensorMap* am = &P.a_maps[sg.a_map];
         const CUtensorMap* bm = P.b_maps + sg.b_map;
@@ -365,7 +407,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         const int pf = P.a_prefetch < P.num_kb ? P.a_prefetch : P.num_kb;
         int nm_tile = 0, nn_tile = 0, nseg_i = 0;
         const bool has_next = tile + (int)gridDim.x < total_tiles;
-        if (pf > 0 && has_next) tile_decode(P, tile + gridDim.x, nm_tile, nn_tile, nseg_i);
+        if (pf > 0 && has_next) tile_decode(P, walk_mt, tile + gridDim.x, nm_tile, nn_tile, nseg_i);
         for (int kb = 0; kb < P.num_kb; ++kb) {
           if (pf > 0) {
             const bool same = kb + pf < P.num_kb;
@@ -398,12 +440,12 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     }
   } else if (warp == 1) {
     // ============================== MMA issuer ==============================
-    if (lane == 0) {
-      const uint32_t idesc = ptx::umma_idesc_bf16(BLOCK_M, block_n);
+    if (lane == 0 && cta_rank == 0) {
+      const uint32_t idesc = ptx::umma_idesc_bf16(PAIR ? 2 * BLOCK_M : BLOCK_M, block_n);
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
+      for (int tile = walker; tile < total_tiles; tile += walk_stride, ++it) {
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
         ptx::mbar_wait_suspend(&bars->tmem_empty[acc], acc_phase ^ 1);
@@ -415,12 +457,16 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
           const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * b_stage_bytes));
 #pragma unroll
-          for (int k = 0; k < BLOCK_K / 16; ++k)
-            ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb | k) != 0);
-          ptx::mma_commit(&bars->empty[stage]);
+          for (int k = 0; k < BLOCK_K / 16; ++k) {
+            if (PAIR) ptx::mma_bf16_cg2(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb | k) != 0);
+            else ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb | k) != 0);
+          }
+          if (PAIR) ptx::mma_commit_cg2(&bars->empty[stage]);      // frees the stage in both CTAs
+          else ptx::mma_commit(&bars->empty[stage]);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
-        ptx::mma_commit(&bars->tmem_full[acc]);
+        if (PAIR) ptx::mma_commit_cg2(&bars->tmem_full[acc]);
+        else ptx::mma_commit(&bars->tmem_full[acc]);
       }
     }
   }
@@ -454,7 +500,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       ri.pos = 0; ri.rs = 1.0f; ri.row_ptr = 0ull;
       ri.m0 = make_float4(0.f, 0.f, 0.f, 0.f); ri.m1 = ri.m0;
       int m_tile, n_tile, seg_i;
-      tile_decode(P, tile, m_tile, n_tile, seg_i);
+      tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
+      if (PAIR) m_tile = 2 * m_tile + (int)cta_rank;
       const TcSeg& sg = P.segs[seg_i];
       const int row = m_tile * BLOCK_M + ew * 32 + lane;
       const int n0 = n_tile * block_n;
@@ -483,12 +530,18 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       return ri;
     };
 
+    // hand an accumulator buffer back to the MMA thread (PAIR: the leader's barrier collects both CTAs' warps)
+    auto release_acc = [&](int acc) {
+      if (PAIR) ptx::mbar_arrive_cluster(ptx::mapa(ptx::smem_u32(&bars->tmem_empty[acc]), 0));
+      else ptx::mbar_arrive(&bars->tmem_empty[acc]);
+    };
     int it = 0;
     RowInfo cur;
-    if ((int)blockIdx.x < total_tiles) cur = fetch(blockIdx.x);
-    for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x, ++it) {
+    if (walker < total_tiles) cur = fetch(walker);
+    for (int tile = walker; tile < total_tiles; tile += walk_stride, ++it) {
       int m_tile, n_tile, seg_i;
-      tile_decode(P, tile, m_tile, n_tile, seg_i);
+      tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
+      if (PAIR) m_tile = 2 * m_tile + (int)cta_rank;
       const TcSeg& sg = P.segs[seg_i];
       const int acc = it & 1;
       const uint32_t acc_phase = (it >> 1) & 1;
@@ -519,7 +572,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // prefetch the next tile's per-row quantities; consumed at the bottom of the loop
       RowInfo nxt = cur;
-      if (tile + (int)gridDim.x < total_tiles) nxt = fetch(tile + gridDim.x);
+      if (tile + walk_stride < total_tiles) nxt = fetch(tile + walk_stride);
 
       if (EPI == EPI_KV && n0 < sg.rope_cols && P.rope_style == SCD_ROPE_HALF && P.head_dim == 128 && block_n == 256 &&
           n_end == 256) {
@@ -530,7 +583,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           else rope_tile_h128_compact<1>(P, t_row, stg, bias, pos, rs, row_ptr, lane);
           ptx::tc_fence_before();
           __syncwarp();
-          if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+          if (lane == 0) release_acc(acc);
           cur = nxt;
           continue;
         }
@@ -538,7 +591,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         else rope_tile_h128<1>(P, t_row, stg, wvec, pos, rs, lane);
         ptx::tc_fence_before();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+        if (lane == 0) release_acc(acc);
         if (grp == 0) rope_tile_h128_copy_out<0>(stg, row_ptr, lane);
         else rope_tile_h128_copy_out<1>(stg, row_ptr, lane);
         cur = nxt;
@@ -571,7 +624,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = 0.0f;
         ptx::tc_fence_before();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+        if (lane == 0) release_acc(acc);
         cur = nxt;
         continue;
       }
@@ -682,7 +735,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           // all TMEM reads of this tile are done: hand the accumulator back before the copy-out
           ptx::tc_fence_before();
           __syncwarp();
-          if (lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
+          if (lane == 0) release_acc(acc);
         } else {
           __syncwarp();
         }
@@ -756,7 +809,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     uint32_t phase = 0;
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
       int m_tile, n_tile_unused, seg_unused;
-      tile_decode(P, tile, m_tile, n_tile_unused, seg_unused);
+      tile_decode(P, walk_mt, tile, m_tile, n_tile_unused, seg_unused);
       const int row = m_tile * BLOCK_M + tr;
       int pos = 0;
       long long slot;
@@ -811,8 +864,13 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
   // ============================== teardown ==============================
   ptx::tc_fence_before();
-  __syncthreads();
-  if (warp == 2) ptx::tmem_dealloc<TMEM_COLS>(tmem_base);
+  if (PAIR) {
+    ptx::cluster_sync();                // neither CTA leaves while the other may still signal its barriers / read its TMEM
+    if (warp == 2) ptx::tmem_dealloc_cg2<TMEM_COLS>(tmem_base);
+  } else {
+    __syncthreads();
+    if (warp == 2) ptx::tmem_dealloc<TMEM_COLS>(tmem_base);
+  }
 }
 
 // ---------------------------------------------------------------------------------
@@ -911,6 +969,9 @@ static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, i
 #ifndef G3_GENERIC
 #define G3_GENERIC 1
 #endif
+#ifndef TC_PAIRS
+#define TC_PAIRS 1
+#endif
 #ifndef TC_A_PREFETCH
 #define TC_A_PREFETCH 4
 #endif
@@ -947,7 +1008,7 @@ scd_status_t tc_supported(const scd_plan_t* p, const scd_layer_desc_t* layers) {
 scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
   const scd_model_desc_t& m = p->model;
   const int nseg = (int)p->segs.size(), np = (int)p->patches.size();
-  std::vector<CUtensorMap> maps((size_t)2 * nseg + 3 * np);
+  std::vector<CUtensorMap> maps((size_t)2 * nseg + 5 * np);   // + per PATCH layer: W2^T and [W_k ; W_v] with 128-row boxes (CTA pairs)
   memset(maps.data(), 0, maps.size() * sizeof(CUtensorMap));
   scd_status_t st;
   for (int i = 0; i < nseg; ++i) {
@@ -961,6 +1022,8 @@ scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
     if ((st = make_b_map(&maps[2 * nseg + 3 * j], pp.w1_t, pp.d_a, pp.r_h, pick_block_n_cover(pp.d_a))) != SCD_OK) return st;
     if ((st = make_b_map(&maps[2 * nseg + 3 * j + 1], pp.w2_t, m.d_model, pp.d_a, pick_block_n_cover(m.d_model))) != SCD_OK) return st;
     if ((st = make_b_map(&maps[2 * nseg + 3 * j + 2], pp.wkv, 2 * p->D, m.d_model, pick_block_n_div(p->D))) != SCD_OK) return st;
+    if ((st = make_b_map(&maps[2 * nseg + 3 * np + 2 * j], pp.w2_t, m.d_model, pp.d_a, 128)) != SCD_OK) return st;
+    if ((st = make_b_map(&maps[2 * nseg + 3 * np + 2 * j + 1], pp.wkv, 2 * p->D, m.d_model, 128)) != SCD_OK) return st;
   }
   void* d = nullptr;
   if (cudaMalloc(&d, maps.size() * sizeof(CUtensorMap) + 64) != cudaSuccess) return fail(SCD_E_NOMEM, "cudaMalloc(tensor maps)");
@@ -980,6 +1043,32 @@ scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
 // ---------------------------------------------------------------------------------
 // launch helper
 // ---------------------------------------------------------------------------------
+// CTA-pair launch: clusters of 2, one cluster per TPC, grid = 2 x min(pair tiles, resident clusters)
+template <int EPI>
+static scd_status_t launch_tc_pair(const scd_plan_t* p, TcParams& P, size_t smem, int pair_tiles, cudaStream_t s) {
+  if (EPI != EPI_U && EPI != EPI_KV) return fail(SCD_E_UNSUPPORTED, "internal: CTA pairs for this epilogue");
+  constexpr int E = (EPI == EPI_U || EPI == EPI_KV) ? EPI : EPI_U;
+  auto kernel = tc_gemm_kernel<E, A_PLAIN, true>;
+  static std::atomic<size_t> configured[SCD_MAX_DEVICES];
+  static std::atomic<int> clusters[SCD_MAX_DEVICES];
+  if (configured[p->device].load(std::memory_order_relaxed) < smem) {
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(pair smem %zu): %s", smem, cudaGetErrorString(e));
+    int n = max_active_clusters(kernel, 384, smem, 2);
+    if (n <= 0) n = p->sm_count / 2;
+    clusters[p->device].store(n, std::memory_order_relaxed);
+    configured[p->device].store(smem, std::memory_order_relaxed);
+  }
+  const int grid = 2 * std::min(pair_tiles, std::min(clusters[p->device].load(std::memory_order_relaxed), p->sm_count / 2));
+  prof_begin(s);
+  launch_pdl(kernel, grid, 384, smem, s, 2, P);
+  prof_end(s, P.prof_id);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel (CTA pairs) launch: %s", cudaGetErrorString(e));
+  count_launch();
+  return SCD_OK;
+}
+
 template <int EPI, int AMODE>
 static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
   P.m_tiles = (P.M + BLOCK_M - 1) / BLOCK_M;
@@ -993,16 +1082,22 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.kv_compact = compact ? 1 : 0;
   P.sub_n = tc_sub_n(EPI, compact);
   P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n, compact, (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2);
-  P.stages = tc_pick_stages(P.block_n, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
+  // CTA pairs (the caller asked and pointed the segments at the 128-row-box B maps): whole 256-column tiles only
+  const bool pair = P.pair && AMODE == A_PLAIN && (EPI == EPI_U || (EPI == EPI_KV && compact)) && P.block_n == 256 && (P.N % 256) == 0;
+  if (P.pair && !pair) return fail(SCD_E_UNSUPPORTED, "internal: CTA-pair launch requested for a shape it does not take");
+  const int b_rows = pair ? P.block_n / 2 : P.block_n;
+  P.stages = tc_pick_stages(b_rows, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
   P.a_prefetch = (EPI == EPI_CODES && !P.a_gather) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
-  P.msb = P.m_tiles;
+  const int walk_mt = pair ? (P.m_tiles + 1) / 2 : P.m_tiles;      // m-tiles of the walk (pair tiles of 256 rows)
+  P.msb = walk_mt;
   if (P.n_tiles > 1) {
-    const long long a_tile_bytes = (long long)BLOCK_M * P.K * 2;
+    const long long a_tile_bytes = (long long)BLOCK_M * P.K * 2 * (pair ? 2 : 1);
     int msb = (int)std::max<long long>(1, (32ll << 20) / a_tile_bytes);
-    if (msb < P.m_tiles) P.msb = msb;
+    if (msb < walk_mt) P.msb = msb;
   }
-  const size_t smem = tc_smem_bytes(P.block_n, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
+  const size_t smem = tc_smem_bytes(b_rows, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
+  if (pair) return launch_tc_pair<EPI>(p, P, smem, P.n_segs * P.n_tiles * walk_mt, s);
   // the attribute belongs to (function, device): cached per instantiation and device ordinal
   static std::atomic<size_t> configured[SCD_MAX_DEVICES];
   if (configured[p->device].load(std::memory_order_relaxed) < smem) {
@@ -1264,6 +1359,10 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
       sg.b_map = 2 * nseg + 3 * (int)(j0 + q) + 1;
     }
     P.prof_id = SCD_PROF_PATCH_GEMM2;
+    if (TC_PAIRS && (d % 256) == 0 && P.block_n == 256 && T > BLOCK_M) {       // CTA pairs: B maps with 128-row boxes
+      P.pair = 1;
+      for (int q = 0; q < g; ++q) P.segs[q].b_map = 2 * nseg + 3 * (int)p->patches.size() + 2 * (int)(j0 + q);
+    }
     if ((st = launch_tc<EPI_U, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     // GEMM-3: [T, d] x [d, 2D] per layer
     fill_common(p, batch, true, false, P, kv->n_blocks);
@@ -1286,6 +1385,10 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
     P.pool_e4m3 = kv->pool_e4m3 ? 1 : 0;
     if (P.pool_e4m3 && !tc_kv_eligible(p, P)) return fail(SCD_E_UNSUPPORTED, "fp8 pools: D must be a multiple of 256");
     const bool long_k = G3_GENERIC && d >= 16 * BLOCK_K && !P.pool_e4m3;   // fp8 pools: only the paged-KV kernel quantises
+    if (TC_PAIRS && long_k && P.block_n == 256 && (P.N % 256) == 0 && m.head_dim == 128 && m.rope_style == SCD_ROPE_HALF && T > BLOCK_M) {
+      P.pair = 1;
+      for (int q = 0; q < g; ++q) P.segs[q].b_map = 2 * nseg + 3 * (int)p->patches.size() + 2 * (int)(j0 + q) + 1;
+    }
     if ((st = (!long_k && tc_kv_eligible(p, P)) ? launch_tc_kv(p, P, s)
                                                                                        : launch_tc<EPI_KV, A_PLAIN>(p, P, s)) != SCD_OK)
       return st;

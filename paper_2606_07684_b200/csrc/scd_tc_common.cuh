@@ -51,6 +51,7 @@ struct TcParams {
   int32_t static_tiles, dyn_begin;    // paged-KV kernel: per-CTA static share, first dynamically claimed tile
   int32_t a_is_codes;                 // paged-KV kernel: A is a code segment (e4m3 codes are widened in shared memory)
   int32_t pool_e4m3;                  // paged-KV kernel: pools are e4m3 bytes + per-(slot, head) fp32 scales
+  int32_t pair;                       // generic kernel, host only: launch as CTA pairs (cta_group::2), B maps have 128-row boxes
   int32_t a_gather;                   // generic kernel: A rows are gathered through P.batch.page_table (paged producer cache)
   long long pool_slots;               // paged epilogues: n_blocks * block_size (slot numbers are kept as int32)
 };
