@@ -63,7 +63,7 @@ static int tc_pick_stages(int b_rows, int num_kb, int stg_warp_bytes, int vec_wa
   const size_t budget = 232448 - 1024 - EPI_WARPS * (stg_warp_bytes + vec_warp_bytes) - sizeof(TcBarriers);
   int st = (int)(budget / (A_STAGE_BYTES + (size_t)b_rows * BLOCK_K * 2));
   st = st > MAX_STAGES ? MAX_STAGES : st;
-  if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty
+  if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty (3, 4 measured: same)
   return st < 2 ? 2 : st;          // odd rings are fine for deRoPE: a k-block pair may straddle the wrap
 }
 
@@ -669,7 +669,11 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
             }
         } else {
           // ---- 32 columns at a time: plain epilogues, or INTERLEAVED RoPE (adjacent pairs) ----
-          const unsigned long long rs2 = f2_pack(rs, rs);
+          // SiLU(v) = v (1/2 + 1/2 tanh(v/2)) = h + h tanh(h) with h = v/2: the halving rides on the scale / bias FMA
+          const bool silu = EPI == EPI_ACT && P.act == SCD_ACT_SILU;
+          const float rsh = silu ? 0.5f * rs : rs;
+          const unsigned long long rs2 = f2_pack(rsh, rsh);
+          const unsigned long long half2 = f2_pack(0.5f, 0.5f);
           for (int c = c0; c < c0 + sub_cols; c += 32) {
             uint32_t r[32];
             ptx::tmem_ld32(t_row + c, r);
@@ -683,18 +687,18 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
                 v[q * 4] = __uint_as_float(r[q * 4]) - m4.x; v[q * 4 + 1] = __uint_as_float(r[q * 4 + 1]) - m4.y;
                 v[q * 4 + 2] = __uint_as_float(r[q * 4 + 2]) - m4.z; v[q * 4 + 3] = __uint_as_float(r[q * 4 + 3]) - m4.w;
               } else {
-                f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4]), __uint_as_float(r[q * 4 + 1])), rs2, f2_pack(m4.x, m4.y)),
-                          v[q * 4], v[q * 4 + 1]);
-                f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4 + 2]), __uint_as_float(r[q * 4 + 3])), rs2, f2_pack(m4.z, m4.w)),
-                          v[q * 4 + 2], v[q * 4 + 3]);
+                unsigned long long b01 = f2_pack(m4.x, m4.y), b23 = f2_pack(m4.z, m4.w);
+                if (silu) { b01 = f2_mul(b01, half2); b23 = f2_mul(b23, half2); }
+                f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4]), __uint_as_float(r[q * 4 + 1])), rs2, b01), v[q * 4], v[q * 4 + 1]);
+                f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4 + 2]), __uint_as_float(r[q * 4 + 3])), rs2, b23), v[q * 4 + 2], v[q * 4 + 3]);
               }
             }
             if (EPI == EPI_ACT && P.act == SCD_ACT_SILU) {
 #pragma unroll
-              for (int i = 0; i < 32; ++i) {      // x sigmoid(x) = x (0.5 + 0.5 tanh(x / 2)): one MUFU op (2^-11 rel.)
+              for (int i = 0; i < 32; ++i) {      // v[i] holds h = x / 2: x sigmoid(x) = h + h tanh(h), one MUFU op (2^-11 rel.)
                 float t;
-                asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(0.5f * v[i]));
-                v[i] *= fmaf(0.5f, t, 0.5f);
+                asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(v[i]));
+                v[i] = fmaf(v[i], t, v[i]);
               }
             }
             if (EPI == EPI_U) {
