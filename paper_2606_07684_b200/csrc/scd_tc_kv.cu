@@ -116,8 +116,12 @@ __device__ __forceinline__ TileCoord tile_coord(const TcParams& P, int tile) {
 // ---------------------------------------------------------------------------------
 constexpr int KV_FIRST_EPI_WARP = 4;
 constexpr int KV_NTHREADS = (KV_FIRST_EPI_WARP + KV_EPI_WARPS) * 32;   // 640
-constexpr int KV_XF_WARPS = 4;                                          // AE4: one code-widening warp per SM sub-partition
-constexpr int KV_NTHREADS_E4 = KV_NTHREADS + KV_XF_WARPS * 32;          // 768
+#ifndef KV_XF_WARPS_N
+#define KV_XF_WARPS_N 8
+#endif
+constexpr int KV_XF_WARPS = KV_XF_WARPS_N;                              // AE4: code-widening warps (two per SM sub-partition)
+constexpr int KV_XF_ITEMS = 512 / (KV_XF_WARPS * 32);                   // 16-code items per thread and k-block
+constexpr int KV_NTHREADS_E4 = KV_NTHREADS + KV_XF_WARPS * 32;          // 896
 
 // DYN: dynamic tile scheduling (hybrid static share + claimed chunks) -- used where tiles are long (PATCH GEMM-3,
 // K = d_model) and SMs drift apart; the REUSE decode keeps the static split, whose epilogue has no registers
@@ -179,7 +183,7 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
   ptx::grid_dep_launch_dependents();    // the next one may start its prologue as SMs free up
 
   if (warp < KV_FIRST_EPI_WARP) {
-    // 128 x 32 + 512 x 112 = 640 x 96 (AE4: 128 x 24 + 512 x 104 + 128 x 40 = 768 x 80): the pool the launch allocated
+    // 128 x 32 + 512 x 112 = 640 x 96 (AE4: 128 x 24 + 512 x 104 + 256 x 32 = 64512 <= 896 x 72): the pool the launch allocated
     if (AE4) ptx::setmaxnreg_dec<24>();
     else ptx::setmaxnreg_dec<32>();
   if (warp == 0) {
@@ -292,10 +296,11 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
   }
   } else if (AE4 && warp >= KV_FIRST_EPI_WARP + KV_EPI_WARPS) {
     // ============================== A transform: e4m3 -> bf16 in shared memory ==============================
-    // 512 items of 16 codes per k-block (row = item / 4, quarter = item % 4), four per thread, read conflict-free from
-    // the raw tile in bytes [8192, 16384) of the stage; all 128 threads meet (the widened rows overwrite the raw
+    // 512 items of 16 codes per k-block (row = item / 4, quarter = item % 4), KV_XF_ITEMS per thread, read conflict-free from
+    // the raw tile in bytes [8192, 16384) of the stage; all widening threads meet (the widened rows overwrite the raw
     // bytes); then each item becomes chunks 2 quarter, 2 quarter + 1 of its row in the 128-byte-swizzled K-major layout.
-    ptx::setmaxnreg_dec<40>();
+    if (KV_XF_WARPS == 4) ptx::setmaxnreg_dec<40>();
+    else ptx::setmaxnreg_dec<32>();
     const int xt = threadIdx.x - (KV_FIRST_EPI_WARP + KV_EPI_WARPS) * 32;
     const uint32_t a_base = ptx::smem_u32(smem_a);
     int stage = 0;
@@ -308,13 +313,13 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
       for (int kb = kb0; kb < kb1; ++kb) {
         ptx::mbar_wait_suspend(&bars->full[stage], phase);
         const uint32_t sb = a_base + (uint32_t)stage * A_STAGE_BYTES;
-        uint4 raw[4];
+        uint4 raw[KV_XF_ITEMS];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) raw[j] = ptx::lds128(sb + A_STAGE_BYTES / 2 + (uint32_t)(xt + 128 * j) * 16);
+        for (int j = 0; j < KV_XF_ITEMS; ++j) raw[j] = ptx::lds128(sb + A_STAGE_BYTES / 2 + (uint32_t)(xt + KV_XF_WARPS * 32 * j) * 16);
         ptx::named_bar_sync(5, KV_XF_WARPS * 32);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const int item = xt + 128 * j, row = item >> 2, qt = item & 3;
+        for (int j = 0; j < KV_XF_ITEMS; ++j) {
+          const int item = xt + KV_XF_WARPS * 32 * j, row = item >> 2, qt = item & 3;
           const uint32_t row_off = (uint32_t)(row >> 3) * 1024 + (uint32_t)(row & 7) * 128;
           const uint32_t w[4] = {raw[j].x, raw[j].y, raw[j].z, raw[j].w};
           uint32_t o[8];
