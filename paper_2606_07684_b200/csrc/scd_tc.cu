@@ -600,7 +600,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // e4m3 codes: the row scale needs the amax over all of N first (tile spans N).  Columns
       // beyond N hold acc = 0 (zero-filled operand rows) and c = 0 (padded vector): no masks needed.
-      float e4_scale = 1.0f;
+      float e4_scale = 1.0f, e4_inv = 1.0f;
       if (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE && has_work) {
         float amax = 0.0f;
         for (int c = 0; c < n_end; c += 32) {
@@ -617,6 +617,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         }
         e4_scale = amax > 0.0f ? amax / 448.0f : 1.0f;
         if (valid && grp == 0) sg.aux[row] = e4_scale;
+        e4_inv = __fdiv_rn(1.0f, e4_scale);     // one division per row; the codes multiply (<= 1.5 ulp of fp32 from z / s)
       }
       float ss_u = 0.0f;
 
@@ -721,8 +722,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
                 uint32_t w[4];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                  w[e] = float2_to_e4m3x2_sat(__fdiv_rn(v[q * 16 + e * 4], e4_scale), __fdiv_rn(v[q * 16 + e * 4 + 1], e4_scale)) |
-                         (float2_to_e4m3x2_sat(__fdiv_rn(v[q * 16 + e * 4 + 2], e4_scale), __fdiv_rn(v[q * 16 + e * 4 + 3], e4_scale)) << 16);
+                  w[e] = float2_to_e4m3x2_sat(v[q * 16 + e * 4] * e4_inv, v[q * 16 + e * 4 + 1] * e4_inv) |
+                         (float2_to_e4m3x2_sat(v[q * 16 + e * 4 + 2] * e4_inv, v[q * 16 + e * 4 + 3] * e4_inv) << 16);
                 }
                 stg_put(stg, pitch, lane, ((c - c0) >> 4) + q, make_uint4(w[0], w[1], w[2], w[3]));
               }
