@@ -8,7 +8,7 @@
 //   1. fit_transpose_kernel   X = [A B] (bf16, [N, W] each) -> Xt [2W, N] K-major, zero-padded; fit_colsum_kernel: fp64
 //                             column sums (means)
 //   2. fit_gram_kernel        G = Xt Xt^T on tcgen05: bf16 x bf16 products are exact in fp32; a TMEM accumulator takes
-//                             at most GRAM_CHUNK_KB k-blocks (2048 samples) and is then added into the fp64 matrix by the
+//                             at most GRAM_CHUNK_KB k-blocks (4096 samples) and is then added into the fp64 matrix by the
 //                             CTA that owns the output tile (deterministic, no atomics), so rounding does not grow with N
 //   3. fit_center_kernel      G <- (G + G^T) / 2 - N mu mu^T   (fp64)
 //   4. jacobi_step_kernel     one-sided (Hestenes) Jacobi on G in fp64, round-robin pair schedule, n/2 CTAs per step,
@@ -75,13 +75,15 @@ __global__ void __launch_bounds__(256) fit_colsum_kernel(const __nv_bfloat16* __
 }
 
 // ---------------------------------------------------------------------------------
-// 3. symmetrise + centre:  Gc[i][j] = (G[i][j] + G[j][i]) / 2 - colsum_i colsum_j / N   (centre != 0)
+// 3. symmetrise + centre:  Gc[i][j] = U[min(i,j)][max(i,j)] - colsum_i colsum_j / N   (centre != 0), U = the two partials' sum
 // ---------------------------------------------------------------------------------
 __global__ void fit_center_kernel(const double* __restrict__ g, const double* __restrict__ colsum, double inv_n, int center, int n,
                                   double* __restrict__ gc) {
   const int j = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
   if (j >= n) return;
-  double v = 0.5 * (g[(size_t)i * n + j] + g[(size_t)j * n + i]);
+  // the Gram kernel fills the tiles that touch the upper triangle, as two split-K partials: entry (min, max) of their sum
+  const size_t at = i <= j ? (size_t)i * n + j : (size_t)j * n + i;
+  double v = g[at] + g[(size_t)n * n + at];
   if (center) v -= colsum[i] * colsum[j] * inv_n;
   gc[(size_t)i * n + j] = v;
 }
@@ -248,14 +250,19 @@ namespace {
 constexpr int GRAM_BLOCK_N = 256;
 constexpr int GRAM_STAGES = 4;
 constexpr int GRAM_B_STAGE_BYTES = GRAM_BLOCK_N * BLOCK_K * 2;        // 32 KB
-constexpr int GRAM_CHUNK_KB = 32;                                      // k-blocks per TMEM accumulation (2048 samples)
-constexpr int GRAM_THREADS = 192;                                      // TMA, MMA, 4 epilogue warps
+constexpr int GRAM_CHUNK_KB = 64;                                      // k-blocks per TMEM accumulation (4096 samples)
+constexpr int GRAM_EPI_WARPS = 8;                                      // two per TMEM lane quadrant (column halves)
+constexpr int GRAM_THREADS = (2 + GRAM_EPI_WARPS) * 32;                // TMA, MMA, epilogue
+constexpr int GRAM_MAX_TILES = 80;                                     // tiles touching the upper triangle at n = 2048: 72
+constexpr int GRAM_SPLIT = 2;                                          // split-K partials (each its own fp64 matrix)
 
 struct GramParams {
   CUtensorMap map_a, map_b;
-  double* g;
+  double* g;             // GRAM_SPLIT matrices [n][n]
   int n;                 // 2W
   int num_kb;            // Np / 64
+  int n_tiles_kept;      // tiles (m, n) with m <= 2 n + 1: G is symmetric, the rest is mirrored afterwards
+  uint8_t tile_m[GRAM_MAX_TILES], tile_n[GRAM_MAX_TILES];
 };
 
 struct __align__(8) GramBarriers {
@@ -273,9 +280,9 @@ __global__ void __launch_bounds__(GRAM_THREADS, 1) fit_gram_kernel(const __grid_
   uint8_t* smem_b = smem + GRAM_STAGES * A_STAGE_BYTES;
   GramBarriers* bars = (GramBarriers*)(smem_b + GRAM_STAGES * GRAM_B_STAGE_BYTES);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int m_tiles = (P.n + BLOCK_M - 1) / BLOCK_M, n_tiles = (P.n + GRAM_BLOCK_N - 1) / GRAM_BLOCK_N;
-  const int total_tiles = m_tiles * n_tiles;
-  const int chunks = (P.num_kb + GRAM_CHUNK_KB - 1) / GRAM_CHUNK_KB;
+  // work item = (kept tile, split-K half): item -> tile item / 2, k-blocks [kb_lo, kb_hi) of half item % 2
+  const int total_items = P.n_tiles_kept * GRAM_SPLIT;
+  const int kb_half = (P.num_kb + GRAM_SPLIT - 1) / GRAM_SPLIT;
 
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < GRAM_STAGES; ++s) {
@@ -284,7 +291,7 @@ __global__ void __launch_bounds__(GRAM_THREADS, 1) fit_gram_kernel(const __grid_
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
-      ptx::mbar_init(&bars->tmem_empty[a], 4);
+      ptx::mbar_init(&bars->tmem_empty[a], GRAM_EPI_WARPS);
     }
     ptx::fence_barrier_init();
   }
@@ -302,9 +309,11 @@ __global__ void __launch_bounds__(GRAM_THREADS, 1) fit_gram_kernel(const __grid_
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        const int m0 = (tile / n_tiles) * BLOCK_M, n0 = (tile % n_tiles) * GRAM_BLOCK_N;
-        for (int kb = 0; kb < P.num_kb; ++kb) {
+      for (int item = blockIdx.x; item < total_items; item += gridDim.x) {
+        const int t = item / GRAM_SPLIT, half = item - t * GRAM_SPLIT;
+        const int m0 = P.tile_m[t] * BLOCK_M, n0 = P.tile_n[t] * GRAM_BLOCK_N;
+        const int kb_lo = half * kb_half, kb_hi = min(P.num_kb, kb_lo + kb_half);
+        for (int kb = kb_lo; kb < kb_hi; ++kb) {
           ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
           ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES + GRAM_B_STAGE_BYTES);
           ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES, &P.map_a, &bars->full[stage], kb * BLOCK_K, m0, 0);
@@ -320,21 +329,23 @@ __global__ void __launch_bounds__(GRAM_THREADS, 1) fit_gram_kernel(const __grid_
       const uint32_t idesc = ptx::umma_idesc_bf16(BLOCK_M, GRAM_BLOCK_N);
       int stage = 0, it = 0;
       uint32_t phase = 0;
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        for (int ch = 0; ch < chunks; ++ch, ++it) {
+      for (int item = blockIdx.x; item < total_items; item += gridDim.x) {
+        const int half = item % GRAM_SPLIT;
+        const int kb_lo = half * kb_half, kb_hi = min(P.num_kb, kb_lo + kb_half);
+        for (int c0 = kb_lo; c0 < kb_hi; c0 += GRAM_CHUNK_KB, ++it) {
           const int acc = it & 1;
           ptx::mbar_wait_suspend(&bars->tmem_empty[acc], ((it >> 1) & 1) ^ 1);
           ptx::tc_fence_after();
           const uint32_t d_tmem = tmem_base + (uint32_t)(acc * GRAM_BLOCK_N);
-          const int kb_end = min(P.num_kb, (ch + 1) * GRAM_CHUNK_KB);
-          for (int kb = ch * GRAM_CHUNK_KB; kb < kb_end; ++kb) {
+          const int c1 = min(kb_hi, c0 + GRAM_CHUNK_KB);
+          for (int kb = c0; kb < c1; ++kb) {
             ptx::mbar_wait_suspend(&bars->full[stage], phase);
             ptx::tc_fence_after();
             const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
             const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * GRAM_B_STAGE_BYTES));
 #pragma unroll
             for (int k = 0; k < BLOCK_K / 16; ++k)
-              ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb > ch * GRAM_CHUNK_KB) || k != 0);
+              ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb > c0) || k != 0);
             ptx::mma_commit(&bars->empty[stage]);
             if (++stage == GRAM_STAGES) { stage = 0; phase ^= 1; }
           }
@@ -343,19 +354,27 @@ __global__ void __launch_bounds__(GRAM_THREADS, 1) fit_gram_kernel(const __grid_
       }
     }
   } else {
-    // ============================== epilogue: G tile (+)= chunk accumulator, fp64 ==============================
+    // ============================== epilogue: partial G tile (+)= chunk accumulator, fp64 ==============================
     const int q = warp & 3;                           // TMEM lane quadrant this warp may read
+    const int ch = (warp - 2) >> 2;                   // column half of the tile
     int it = 0;
-    for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-      const int m0 = (tile / n_tiles) * BLOCK_M, n0 = (tile % n_tiles) * GRAM_BLOCK_N;
+    for (int item = blockIdx.x; item < total_items; item += gridDim.x) {
+      const int t = item / GRAM_SPLIT, half = item - t * GRAM_SPLIT;
+      const int m0 = P.tile_m[t] * BLOCK_M, n0 = P.tile_n[t] * GRAM_BLOCK_N;
+      const int kb_lo = half * kb_half, kb_hi = min(P.num_kb, kb_lo + kb_half);
       const int row = m0 + q * 32 + lane;
-      double* grow = P.g + (size_t)row * P.n + n0;
-      for (int ch = 0; ch < chunks; ++ch, ++it) {
+      double* grow = P.g + (size_t)half * P.n * P.n + (size_t)row * P.n + n0;
+      if (kb_lo >= kb_hi) {                           // an empty half (fewer k-blocks than halves): its partial is zero
+        if (row < P.n)
+          for (int c = ch * 128; c < ch * 128 + 128 && n0 + c < P.n; ++c) grow[c] = 0.0;
+        continue;
+      }
+      for (int c0 = kb_lo; c0 < kb_hi; c0 += GRAM_CHUNK_KB, ++it) {
         const int acc = it & 1;
         ptx::mbar_wait_suspend(&bars->tmem_full[acc], (it >> 1) & 1);
         ptx::tc_fence_after();
         const uint32_t t_row = tmem_base + (uint32_t)(acc * GRAM_BLOCK_N) + ((uint32_t)(q * 32) << 16);
-        for (int c = 0; c < GRAM_BLOCK_N && n0 + c < P.n; c += 32) {
+        for (int c = ch * 128; c < ch * 128 + 128 && n0 + c < P.n; c += 32) {
           uint32_t r[32];
           ptx::tmem_ld32(t_row + c, r);
           ptx::tmem_ld_wait();
@@ -363,7 +382,7 @@ __global__ void __launch_bounds__(GRAM_THREADS, 1) fit_gram_kernel(const __grid_
 #pragma unroll
             for (int j = 0; j < 32; j += 2) {
               if (n0 + c + j < P.n) {               // n is even: columns j, j + 1 are valid together
-                double2 v = ch ? *reinterpret_cast<double2*>(grow + c + j) : make_double2(0.0, 0.0);
+                double2 v = c0 > kb_lo ? *reinterpret_cast<double2*>(grow + c + j) : make_double2(0.0, 0.0);
                 v.x += (double)__uint_as_float(r[j]);
                 v.y += (double)__uint_as_float(r[j + 1]);
                 *reinterpret_cast<double2*>(grow + c + j) = v;
@@ -406,7 +425,7 @@ FitLayout fit_layout(int W, int r, long long N) {
   size_t at = 0;
   auto take = [&](size_t bytes) { size_t o = at; at = align_up(at + bytes, 256); return o; };
   L.xt = take(n * (size_t)L.Np * 2);
-  L.g = take(n * n * 8);
+  L.g = take(n * n * 8 * GRAM_SPLIT);    // split-K partials of the Gram kernel; the first is reused for the centred matrix
   L.u = take(n * n * 8);                 // centred Gram matrix, then the Jacobi iterate
   L.ga = take((size_t)W * W * 8);
   L.colsum = take(n * 8);
@@ -514,6 +533,15 @@ extern "C" scd_status_t scd_fit_reuse(const scd_fit_desc_t* d, const void* a, co
     P.g = g;
     P.n = n;
     P.num_kb = (int)(L.Np / BLOCK_K);
+    const int mt = (n + BLOCK_M - 1) / BLOCK_M, nt = (n + GRAM_BLOCK_N - 1) / GRAM_BLOCK_N;
+    P.n_tiles_kept = 0;
+    for (int tn = 0; tn < nt; ++tn)
+      for (int tm = 0; tm < mt && tm <= 2 * tn + 1; ++tm) {
+        if (P.n_tiles_kept >= GRAM_MAX_TILES) return fail(SCD_E_UNSUPPORTED, "fit: too many Gram tiles");
+        P.tile_m[P.n_tiles_kept] = (uint8_t)tm;
+        P.tile_n[P.n_tiles_kept] = (uint8_t)tn;
+        ++P.n_tiles_kept;
+      }
     int dev = 0, sms = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -523,9 +551,9 @@ extern "C" scd_status_t scd_fit_reuse(const scd_fit_desc_t* d, const void* a, co
       if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(gram smem): %s", cudaGetErrorString(e));
       configured[dev].store(1);
     }
-    const int tiles = ((n + BLOCK_M - 1) / BLOCK_M) * ((n + GRAM_BLOCK_N - 1) / GRAM_BLOCK_N);
+    const int items = P.n_tiles_kept * GRAM_SPLIT;
     prof_begin(s);
-    fit_gram_kernel<<<std::min(tiles, std::max(sms, 1)), GRAM_THREADS, GRAM_SMEM, s>>>(P);
+    fit_gram_kernel<<<std::min(items, std::max(sms, 1)), GRAM_THREADS, GRAM_SMEM, s>>>(P);
     prof_end(s, SCD_PROF_FIT_GRAM);
     FIT_LAUNCH_CHECK("fit_gram_kernel");
   }
