@@ -242,7 +242,7 @@ def run_extras(prob, cfg, k, v, peaks, flush, stream, iters=10):
             h_src[l] = prob._bench_h[l]
         p_ms, p_best = timed(lambda: prob.encode(k, v, h_src, src_page_table=prob.batch.page_table, src_n_blocks=T // cfg.block_size))
         e_ms, e_best = timed(lambda: prob.encode(k, v, h_src))
-        out["encode_paged_source"] = {"packed_ms": e_ms, "paged_ms": p_ms, "note": "K_A / V_A gathered through a producer page table (TMA tile::gather4)"}
+        out["encode_paged_source"] = {"packed_ms": e_ms, "paged_ms": p_ms, "note": "K_A / V_A read through a producer page table (TMA: one 16-row box per page where rows align with pages, tile::gather4 otherwise)"}
     # ---- REUSE decode into fp8 pools (e4m3 bytes + one fp32 scale per (slot, head))
     if cfg.head_dim == 128 and D % 256 == 0:
         nb = prob.batch.n_blocks
