@@ -438,10 +438,10 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
       // address of this lane's 16 bytes in slot 0 of the tile's pool columns; a row adds slot * row_stride
       const unsigned long long tile_base = (unsigned long long)(to1 ? sg.out1 : sg.out0) +
                                            (unsigned long long)(to1 ? n0 - P.split : n0) * (P8 ? 1ull : 2ull) +
-                                           (unsigned long long)lane * (P8 ? 8ull : 16ull);
+                                           (unsigned long long)(P8 ? (lane & 15) : lane) * 16ull;
       // fp8 pools: scale of this lane's head = [slot][head]
       float* scale_base = nullptr;
-      if (P8) scale_base = (to1 ? sg.scale1 : sg.scale0) + ((to1 ? n0 - P.split : n0) >> 7) + (lane >> 4);
+      if (P8) scale_base = (to1 ? sg.scale1 : sg.scale0) + ((to1 ? n0 - P.split : n0) >> 7) + ((lane >> 3) & 1);
       const uint32_t scale_stride = (uint32_t)(P.pool_width >> 7);
 
       // this warp's slice of the tile's mean / bias: wvec[16 * run + i]
@@ -526,7 +526,36 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
       ptx::tc_fence_before();
       ptx::named_bar_sync(bar_id, 128);
       if (g == 0 && lane == 0) ptx::mbar_arrive(&bars->tmem_empty[acc]);
-      {
+      if (P8) {
+        // fp8 pools: a warp pass covers TWO rows -- lanes 0-15 the even row, 16-31 the odd one -- and a lane converts 16
+        // columns (two staged chunks) into one 16-byte store, so the store instructions carry full 16-byte lanes as in
+        // the bf16 path.  A head is 8 lanes: its amax takes 3 shuffles; s = amax / 448, bytes = e4m3(x * (1 / s)).
+        const int hl = lane & 15;
+#pragma unroll
+        for (int p2 = 0; p2 < 4; ++p2) {
+          const int r = 8 * g + 2 * p2 + (lane >> 4);
+          int slot;
+          asm volatile("ld.shared.b32 %0, [%1];" : "=r"(slot) : "r"(wslot + r * 4) : "memory");
+          const uint4 x0 = ptx::lds128(qstg_addr(stg, r, 2 * hl)), x1 = ptx::lds128(qstg_addr(stg, r, 2 * hl + 1));
+          const uint32_t w[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+          float a = 0.0f;
+#pragma unroll
+          for (int j = 0; j < 8; ++j) a = fmaxf(a, fmaxf(fabsf(__uint_as_float(w[j] << 16)), fabsf(__uint_as_float(w[j] & 0xffff0000u))));
+#pragma unroll
+          for (int o = 1; o < 8; o <<= 1) a = fmaxf(a, __shfl_xor_sync(0xffffffffu, a, o));
+          const float sc = a > 0.0f ? __fdiv_rn(a, 448.0f) : 1.0f;
+          const float inv = __fdiv_rn(1.0f, sc);
+          uint32_t o4[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j)
+            o4[j] = float2_to_e4m3x2_sat(__fmul_rn(__uint_as_float(w[2 * j] << 16), inv), __fmul_rn(__uint_as_float(w[2 * j] & 0xffff0000u), inv)) |
+                    (float2_to_e4m3x2_sat(__fmul_rn(__uint_as_float(w[2 * j + 1] << 16), inv), __fmul_rn(__uint_as_float(w[2 * j + 1] & 0xffff0000u), inv)) << 16);
+          if (slot >= 0) {
+            ptx::stg128_cs(tile_base + (unsigned long long)(uint32_t)slot * row_stride, make_uint4(o4[0], o4[1], o4[2], o4[3]));
+            if ((lane & 7) == 0) scale_base[(size_t)(uint32_t)slot * scale_stride] = sc;
+          }
+        }
+      } else {
         uint4 v[8];
         int sl[8];
 #pragma unroll
@@ -535,36 +564,9 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
           asm volatile("ld.shared.b32 %0, [%1];" : "=r"(sl[i]) : "r"(wslot + r * 4) : "memory");
           v[i] = ptx::lds128(qstg_addr(stg, r, lane));
         }
-        if (P8) {
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const uint32_t w[4] = {v[i].x, v[i].y, v[i].z, v[i].w};
-            float f[8];
-#pragma unroll
-            for (int j = 0; j < 4; ++j) { f[2 * j] = __uint_as_float(w[j] << 16); f[2 * j + 1] = __uint_as_float(w[j] & 0xffff0000u); }
-            float amax = 0.0f;
-#pragma unroll
-            for (int j = 0; j < 8; ++j) amax = fmaxf(amax, fabsf(f[j]));
-#pragma unroll
-            for (int o = 1; o < 16; o <<= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, o));   // the head's 16 lanes
-            const float sc = amax > 0.0f ? __fdiv_rn(amax, 448.0f) : 1.0f;
-            const float inv = __fdiv_rn(1.0f, sc);
-            uint32_t b0 = 0, b1 = 0;
-#pragma unroll
-            for (int j = 0; j < 2; ++j) {
-              b0 |= float2_to_e4m3x2_sat(__fmul_rn(f[2 * j], inv), __fmul_rn(f[2 * j + 1], inv)) << (16 * j);
-              b1 |= float2_to_e4m3x2_sat(__fmul_rn(f[4 + 2 * j], inv), __fmul_rn(f[5 + 2 * j], inv)) << (16 * j);
-            }
-            if (sl[i] >= 0) {
-              asm volatile("st.global.cs.v2.b32 [%0], {%1, %2};" ::"l"(tile_base + (unsigned long long)(uint32_t)sl[i] * row_stride), "r"(b0), "r"(b1) : "memory");
-              if ((lane & 15) == 0) scale_base[(size_t)(uint32_t)sl[i] * scale_stride] = sc;
-            }
-          }
-        } else {
 #pragma unroll
         for (int i = 0; i < 8; ++i)
           if (sl[i] >= 0) ptx::stg128_cs(tile_base + (unsigned long long)(uint32_t)sl[i] * row_stride, v[i]);
-        }
       }
       cur = nxt;
       tc = tn;
