@@ -990,6 +990,9 @@ static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, i
 #ifndef TC_PAIRS
 #define TC_PAIRS 1
 #endif
+#ifndef TC_ENC_PAIRS
+#define TC_ENC_PAIRS 1
+#endif
 #ifndef TC_A_PREFETCH
 #define TC_A_PREFETCH 4
 #endif
@@ -1026,12 +1029,14 @@ scd_status_t tc_supported(const scd_plan_t* p, const scd_layer_desc_t* layers) {
 scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
   const scd_model_desc_t& m = p->model;
   const int nseg = (int)p->segs.size(), np = (int)p->patches.size();
-  std::vector<CUtensorMap> maps((size_t)2 * nseg + 5 * np);   // + per PATCH layer: W2^T and [W_k ; W_v] with 128-row boxes (CTA pairs)
+  // + per PATCH layer: W2^T and [W_k ; W_v] with 128-row boxes, + per segment the encoder with half-tile boxes (CTA pairs)
+  std::vector<CUtensorMap> maps((size_t)3 * nseg + 5 * np);
   memset(maps.data(), 0, maps.size() * sizeof(CUtensorMap));
   scd_status_t st;
   for (int i = 0; i < nseg; ++i) {
     const SegPlan& sp = p->segs[i];
     if ((st = make_b_map(&maps[i], sp.enc_t, sp.rank, sp.width, pick_block_n_cover(sp.rank))) != SCD_OK) return st;
+    if ((st = make_b_map(&maps[2 * nseg + 5 * np + i], sp.enc_t, sp.rank, sp.width, pick_block_n_cover(sp.rank) / 2)) != SCD_OK) return st;
     if (sp.dec_t)
       if ((st = make_b_map(&maps[nseg + i], sp.dec_t, p->D, sp.rank, pick_block_n_div(p->D))) != SCD_OK) return st;
   }
@@ -1064,8 +1069,8 @@ scd_status_t tc_plan_init(scd_plan_t* p, cudaStream_t s) {
 // CTA-pair launch: clusters of 2, one cluster per TPC, grid = 2 x min(pair tiles, resident clusters)
 template <int EPI>
 static scd_status_t launch_tc_pair(const scd_plan_t* p, TcParams& P, size_t smem, int pair_tiles, cudaStream_t s) {
-  if (EPI != EPI_U && EPI != EPI_KV) return fail(SCD_E_UNSUPPORTED, "internal: CTA pairs for this epilogue");
-  constexpr int E = (EPI == EPI_U || EPI == EPI_KV) ? EPI : EPI_U;
+  if (EPI != EPI_U && EPI != EPI_KV && EPI != EPI_CODES) return fail(SCD_E_UNSUPPORTED, "internal: CTA pairs for this epilogue");
+  constexpr int E = (EPI == EPI_U || EPI == EPI_KV || EPI == EPI_CODES) ? EPI : EPI_U;
   auto kernel = tc_gemm_kernel<E, A_PLAIN, true>;
   static std::atomic<size_t> configured[SCD_MAX_DEVICES];
   static std::atomic<int> clusters[SCD_MAX_DEVICES];
@@ -1101,7 +1106,9 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   P.sub_n = tc_sub_n(EPI, compact);
   P.stg_warp_bytes = tc_stg_warp_bytes(EPI, P.block_n, compact, (EPI == EPI_CODES && P.code_dtype == SCD_E4M3_ROWSCALE) ? 1 : 2);
   // CTA pairs (the caller asked and pointed the segments at the 128-row-box B maps): whole 256-column tiles only
-  const bool pair = P.pair && AMODE == A_PLAIN && (EPI == EPI_U || (EPI == EPI_KV && compact)) && P.block_n == 256 && (P.N % 256) == 0;
+  const bool pair = P.pair && AMODE == A_PLAIN &&
+                    (((EPI == EPI_U || (EPI == EPI_KV && compact)) && P.block_n == 256 && (P.N % 256) == 0) ||
+                     (EPI == EPI_CODES && (P.block_n % 32) == 0));
   if (P.pair && !pair) return fail(SCD_E_UNSUPPORTED, "internal: CTA-pair launch requested for a shape it does not take");
   const int b_rows = pair ? P.block_n / 2 : P.block_n;
   P.stages = tc_pick_stages(b_rows, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
@@ -1239,6 +1246,12 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
         return fail(SCD_E_UNSUPPORTED, "deRoPE-on-load implements the HALF pairing only on the bf16 path");
       st = launch_tc<EPI_CODES, A_DEROPE>(p, P, s);
     } else {
+      // wide ranks (256-column tiles): CTA pairs, half of the W_enc^T tile per CTA (config 4: V 0.453 -> 0.420 ms, H 0.258 ->
+      // 0.220 ms; at r = 128 the plain kernel with its L2 prefetch of the A stream is as fast: 0.098 vs 0.101 ms)
+      if (TC_ENC_PAIRS && P.block_n == 256 && !gather && P.a_kb_per_head == 0 && T > BLOCK_M) {
+        P.pair = 1;
+        for (size_t q = i; q < j; ++q) P.segs[q - i].b_map = 2 * (int)nseg + 5 * (int)p->patches.size() + p->segs[q].seg_index;
+      }
       st = launch_tc<EPI_CODES, A_PLAIN>(p, P, s);
     }
     if (st != SCD_OK) return st;
