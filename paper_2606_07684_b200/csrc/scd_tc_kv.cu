@@ -19,6 +19,9 @@
 
 #include "scd_tc_common.cuh"
 
+#ifndef KV_ARES
+#define KV_ARES 1
+#endif
 #ifndef KV_STATIC_PCT
 #define KV_STATIC_PCT 60
 #endif
@@ -40,12 +43,23 @@ struct __align__(8) KvBarriers {
   uint64_t tmem_full[2], tmem_empty[2];
   uint64_t sched_full[4], sched_empty[4];                    // chunk ring (KV_SCHED_SLOTS)
   int32_t sched_begin[4], sched_end[4];                      // tile range of the entry; begin < 0 = no more work
+  uint64_t a_full[4], a_ready[4], a_empty[4];                // ARES: the resident code tile's k-block slots
   uint32_t tmem_base;
 };
 constexpr int KV_SCHED_SLOTS = 4;
 
 size_t kv_smem_bytes(int stages) {
   return 1024 + (size_t)stages * (A_STAGE_BYTES + KV_B_STAGE_BYTES) + KV_STG_BYTES + KV_VEC_BYTES + KV_SLOT_BYTES + sizeof(KvBarriers);
+}
+// ARES (code tile resident across the n-tiles of its (m-tile, segment)): num_kb slots of 16 KB + a ring of basis stages
+size_t kva_smem_bytes(int b_stages, int num_kb) {
+  return 1024 + (size_t)num_kb * A_STAGE_BYTES + (size_t)b_stages * KV_B_STAGE_BYTES + KV_STG_BYTES + KV_VEC_BYTES + KV_SLOT_BYTES +
+         sizeof(KvBarriers);
+}
+int kva_pick_stages(int num_kb) {
+  const size_t budget = 232448 - 1024 - KV_STG_BYTES - KV_VEC_BYTES - KV_SLOT_BYTES - sizeof(KvBarriers) - (size_t)num_kb * A_STAGE_BYTES;
+  int st = (int)(budget / KV_B_STAGE_BYTES);
+  return st > MAX_STAGES ? MAX_STAGES : st;
 }
 int kv_pick_stages(int num_kb) {
   const size_t budget = 232448 - 1024 - KV_STG_BYTES - KV_VEC_BYTES - KV_SLOT_BYTES - sizeof(KvBarriers);
@@ -135,15 +149,20 @@ constexpr int KV_NTHREADS_E4 = KV_NTHREADS + KV_XF_WARPS * 32;          // 896
 // P8: the pools are e4m3 bytes with one fp32 scale per (slot, head) (fp8 pools, scd.h): the copy-out, which holds a
 // complete bf16 row segment of two heads per warp pass, takes the head's amax over its 16 lanes, and stores 8 bytes per
 // lane plus the scale.
-template <bool DYN, bool SCALED, bool AE4, bool P8>
+// ARES (e4m3 codes, K <= 256): the code tile of an (m-tile, segment) serves all of its n-tiles, which are consecutive in
+// the walk; widening it once per n-tile is what bounds the e4m3 decode (profiles/r02_decode_history.md).  Here its k-blocks
+// get slots of their own: loaded and widened ONCE when the CTA enters the (m-tile, segment), released by the MMAs of the last
+// n-tile; only the basis tiles go through the ring.
+template <bool DYN, bool SCALED, bool AE4, bool P8, bool ARES = false>
 __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
   static_assert(!AE4 || (SCALED && !DYN), "e4m3 codes carry row scales; static split");
+  static_assert(!ARES || AE4, "resident code tiles: e4m3 codes only");
   static_assert(!P8 || SCALED, "fp8 pools are built on the scaled variants only");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
   uint8_t* smem_a = smem;
-  uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
+  uint8_t* smem_b = smem + (ARES ? P.num_kb : STAGES) * A_STAGE_BYTES;      // ARES: STAGES counts basis stages only
   uint8_t* smem_stg = smem_b + STAGES * KV_B_STAGE_BYTES;
   uint8_t* smem_vec = smem_stg + KV_STG_BYTES;
   uint8_t* smem_slot = smem_vec + KV_VEC_BYTES;
@@ -164,6 +183,11 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
       ptx::mbar_init(&bars->tmem_empty[a], 4);          // one arrival per lane quadrant
+    }
+    for (int a = 0; a < 4; ++a) {
+      ptx::mbar_init(&bars->a_full[a], 1);
+      ptx::mbar_init(&bars->a_ready[a], KV_XF_WARPS * 32);
+      ptx::mbar_init(&bars->a_empty[a], 1);
     }
     for (int a = 0; a < KV_SCHED_SLOTS; ++a) {
       ptx::mbar_init(&bars->sched_full[a], 1);
@@ -188,6 +212,30 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
     else ptx::setmaxnreg_dec<32>();
   if (warp == 0) {
     // ============================== TMA producer ==============================
+    if (ARES) {
+      if (lane == 0) {
+        int stage = 0;
+        uint32_t phase = 0, groups = 0;                       // groups = (m-tile, segment) code tiles started so far
+        TileCoord tc = tile_coord<false>(P, s_begin);
+        for (int tile = s_begin; tile < s_end; ++tile, tile_next<false>(P, tc)) {
+          const TcSeg& sg = P.segs[tc.seg];
+          const bool grp_first = tile == s_begin || tc.n_tile == 0;
+          for (int kb = 0; kb < P.num_kb; ++kb) {
+            if (grp_first) {                                   // the code tile's k-block, once its slot has been released
+              if (groups > 0) ptx::mbar_wait_suspend(&bars->a_empty[kb], (groups - 1) & 1);
+              ptx::mbar_expect_tx(&bars->a_full[kb], A_STAGE_BYTES / 2);
+              ptx::tma_load_3d(smem_a + kb * A_STAGE_BYTES + A_STAGE_BYTES / 2, &P.a_maps[sg.a_map], &bars->a_full[kb], kb * BLOCK_K,
+                               tc.m_tile * BLOCK_M, sg.a_z);
+            }
+            ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
+            ptx::mbar_expect_tx(&bars->full[stage], KV_B_STAGE_BYTES);
+            ptx::tma_load_2d(smem_b + stage * KV_B_STAGE_BYTES, P.b_maps + sg.b_map, &bars->full[stage], kb * BLOCK_K, tc.n_tile * KV_BLOCK_N);
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+          if (grp_first) ++groups;
+        }
+      }
+    } else
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
@@ -249,6 +297,38 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
     }
   } else if (warp == 1) {
     // ============================== MMA issuer ==============================
+    if (ARES) {
+      if (lane == 0) {
+        const uint32_t idesc = ptx::umma_idesc_bf16(BLOCK_M, KV_BLOCK_N);
+        int stage = 0, it = 0;
+        uint32_t phase = 0, groups = 0;                       // groups completed
+        int n_tile = s_begin % P.n_tiles;
+        for (int tile = s_begin; tile < s_end; ++tile, ++it) {
+          const bool grp_first = tile == s_begin || n_tile == 0;
+          const bool grp_last = tile == s_end - 1 || n_tile == P.n_tiles - 1;
+          if (++n_tile == P.n_tiles) n_tile = 0;
+          const int acc = it & 1;
+          ptx::mbar_wait_suspend(&bars->tmem_empty[acc], ((it >> 1) & 1) ^ 1);
+          ptx::tc_fence_after();
+          const uint32_t d_tmem = tmem_base + (uint32_t)(acc * KV_BLOCK_N);
+          for (int kb = 0; kb < P.num_kb; ++kb) {
+            if (grp_first) ptx::mbar_wait_suspend(&bars->a_ready[kb], groups & 1);      // landed and widened, once per group
+            ptx::mbar_wait_suspend(&bars->full[stage], phase);
+            ptx::tc_fence_after();
+            const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + kb * A_STAGE_BYTES));
+            const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + stage * KV_B_STAGE_BYTES));
+#pragma unroll
+            for (int k = 0; k < BLOCK_K / 16; ++k)
+              ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb | k) != 0);
+            ptx::mma_commit(&bars->empty[stage]);
+            if (grp_last) ptx::mma_commit(&bars->a_empty[kb]);                           // the slot may take the next code tile
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+          ptx::mma_commit(&bars->tmem_full[acc]);
+          if (grp_last) ++groups;
+        }
+      }
+    } else
     if (lane == 0) {
       const uint32_t idesc = ptx::umma_idesc_bf16(BLOCK_M, KV_BLOCK_N);
       int stage = 0;
@@ -306,12 +386,16 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
     int stage = 0;
     uint32_t phase = 0;
     int n_tile = s_begin % P.n_tiles;
+    uint32_t groups = 0;
     for (int tile = s_begin; tile < s_end; ++tile) {
       int kb0, kb1;
       tile_kb_range(P, n_tile, kb0, kb1);
+      const bool grp_first = tile == s_begin || n_tile == 0;
       if (++n_tile == P.n_tiles) n_tile = 0;
+      if (ARES && !grp_first) continue;                       // the code tile of this (m-tile, segment) is already widened
       for (int kb = kb0; kb < kb1; ++kb) {
-        ptx::mbar_wait_suspend(&bars->full[stage], phase);
+        if (ARES) { stage = kb; phase = groups & 1; }
+        ptx::mbar_wait_suspend(ARES ? &bars->a_full[kb] : &bars->full[stage], phase);
         const uint32_t sb = a_base + (uint32_t)stage * A_STAGE_BYTES;
         uint4 raw[KV_XF_ITEMS];
 #pragma unroll
@@ -332,9 +416,14 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
           ptx::sts128(sb + row_off + (uint32_t)(((2 * qt + 1) ^ (row & 7)) << 4), make_uint4(o[4], o[5], o[6], o[7]));
         }
         ptx::fence_proxy_async_smem();
-        ptx::mbar_arrive(&bars->ready[stage]);
-        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        if (ARES) {
+          ptx::mbar_arrive(&bars->a_ready[kb]);
+        } else {
+          ptx::mbar_arrive(&bars->ready[stage]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
       }
+      if (ARES) ++groups;
     }
   } else {
     // ============================== epilogue ==============================
@@ -611,6 +700,25 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
     configured[p->device].store(smem, std::memory_order_relaxed);
+  }
+  // e4m3 codes of rank <= 256 on bf16 pools: the code tile stays resident across its n-tiles
+  if (KV_ARES && P.code_dtype == SCD_E4M3_ROWSCALE && P.a_is_codes && !P.pool_e4m3 && P.head_rank == 0 && P.num_kb <= 4 && P.n_tiles > 1) {
+    P.stages = kva_pick_stages(P.num_kb);
+    const size_t smem_a_ = kva_smem_bytes(P.stages, P.num_kb);
+    static std::atomic<size_t> conf_a[SCD_MAX_DEVICES];
+    if (conf_a[p->device].load(std::memory_order_relaxed) < smem_a_) {
+      cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false, true, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a_);
+      if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv resident smem %zu): %s", smem_a_, cudaGetErrorString(e));
+      conf_a[p->device].store(smem_a_, std::memory_order_relaxed);
+    }
+    if ((long long)P.pool_slots >= (1ll << 31)) return fail(SCD_E_UNSUPPORTED, "pools of more than 2^31 slots");
+    prof_begin(s);
+    launch_pdl(tc_kv_kernel<false, true, true, false, true>, std::min(total, p->sm_count), KV_NTHREADS_E4, smem_a_, s, 1, P);
+    prof_end(s, P.prof_id);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_kv_kernel (resident code tile) launch: %s", cudaGetErrorString(e));
+    count_launch();
+    return SCD_OK;
   }
   const int grid = std::min(total, p->sm_count);
   // long tiles (K = d_model: PATCH GEMM-3): KV_STATIC_PCT % of an even split is owned statically, the rest is
