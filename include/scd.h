@@ -303,6 +303,10 @@ int32_t scd_profile_fetch(float* ms /* HOST [max] */, int32_t* kernel_id /* HOST
 /* Thread-local message for the last non-OK status returned on this thread ("" if none). */
 const char* scd_last_error(void);
 
+/* sizeof() of the ABI structs as this library was compiled (0 model, 1 layer, 2 batch, 3 src, 4 paged_kv, 5 int4 desc,
+ * 6 fit desc; -1 otherwise): lets a binding verify its struct layouts before the first call. */
+int32_t scd_struct_size(int32_t which);
+
 /* Library version string. */
 const char* scd_version(void);
 

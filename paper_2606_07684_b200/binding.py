@@ -35,7 +35,7 @@ EXPORTS = ["scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segm
            "scd_patch_layers", "scd_last_launch_count", "scd_profile_enable",
            "scd_profile_fetch", "scd_last_error", "scd_version",
            "scd_int4_layout", "scd_int4_quantize", "scd_int4_dequantize_paged",
-           "scd_fit_query", "scd_fit_reuse"]
+           "scd_fit_query", "scd_fit_reuse", "scd_struct_size"]
 
 
 class ModelDesc(C.Structure):
@@ -126,6 +126,12 @@ def _load() -> C.CDLL:
     lib.scd_profile_enable.restype = C.c_int
     lib.scd_profile_fetch.argtypes = [C.POINTER(C.c_float), pi32, i32]
     lib.scd_profile_fetch.restype = C.c_int32
+    lib.scd_struct_size.argtypes = [i32]
+    lib.scd_struct_size.restype = C.c_int32
+    for which, cls in enumerate((ModelDesc, LayerDesc, BatchDesc, SrcDesc, PagedKV, Int4Desc, FitDesc)):
+        if lib.scd_struct_size(which) != C.sizeof(cls):
+            raise ImportError(f"libscd.so and binding.py disagree on the layout of {cls.__name__}: "
+                              f"{lib.scd_struct_size(which)} vs {C.sizeof(cls)} bytes (rebuild the library)")
     lib.scd_last_error.restype = C.c_char_p
     lib.scd_version.restype = C.c_char_p
     return lib

@@ -374,6 +374,18 @@ extern "C" {
 
 const char* scd_last_error(void) { return g_err; }
 int32_t scd_last_launch_count(void) { return g_launches; }
+int32_t scd_struct_size(int32_t which) {
+  switch (which) {
+    case 0: return (int32_t)sizeof(scd_model_desc_t);
+    case 1: return (int32_t)sizeof(scd_layer_desc_t);
+    case 2: return (int32_t)sizeof(scd_batch_t);
+    case 3: return (int32_t)sizeof(scd_src_t);
+    case 4: return (int32_t)sizeof(scd_paged_kv_t);
+    case 5: return (int32_t)sizeof(scd_int4_desc_t);
+    case 6: return (int32_t)sizeof(scd_fit_desc_t);
+    default: return -1;
+  }
+}
 const char* scd_version(void) { return "scd-b200 0.1 (sm_100a)"; }
 
 scd_status_t scd_profile_enable(int32_t on) {

@@ -166,3 +166,11 @@ def test_int4_layout_matches_oracle_payload_and_rejects_bad_groups(B):
     for bad in (B.Int4Desc(8, 128, 16, 16), B.Int4Desc(8, 64, 16, 128), B.Int4Desc(0, 128, 16, 32)):
         with pytest.raises(B.ScdError):
             B.scd_int4_layout(bad, 10, 1)
+
+
+def test_struct_layouts_agree_with_the_library(B):
+    """The ctypes structs of the binding have the sizes the C compiler gave the ABI structs (scd_struct_size)."""
+    import ctypes as C
+    for which, cls in enumerate((B.ModelDesc, B.LayerDesc, B.BatchDesc, B.SrcDesc, B.PagedKV, B.Int4Desc, B.FitDesc)):
+        assert B.lib.scd_struct_size(which) == C.sizeof(cls), cls.__name__
+    assert B.lib.scd_struct_size(99) == -1
