@@ -174,3 +174,20 @@ def test_struct_layouts_agree_with_the_library(B):
     for which, cls in enumerate((B.ModelDesc, B.LayerDesc, B.BatchDesc, B.SrcDesc, B.PagedKV, B.Int4Desc, B.FitDesc)):
         assert B.lib.scd_struct_size(which) == C.sizeof(cls), cls.__name__
     assert B.lib.scd_struct_size(99) == -1
+
+
+def test_fit_query_is_pure_host_arithmetic(B):
+    """scd_fit_query validates the descriptor and sizes the workspace without touching a device: the K-major copy of
+    X = [A B] (2 W x ceil(N / 64) * 64 bf16) dominates; bad descriptors come back with the documented statuses."""
+    d = B.FitDesc(1024, 128, 1, 1e-3, B.SCD_BF16, B.SCD_BF16)
+    ws = B.scd_fit_query(d, 100000)
+    xt = 2 * 1024 * ((100000 + 63) // 64 * 64) * 2
+    assert xt < ws < xt + 200 * (1 << 20) and B.scd_fit_query(d, 1) < B.scd_fit_query(d, 100000)
+    for desc, status in ((B.FitDesc(60, 8, 0, 1e-3, B.SCD_BF16, B.SCD_F32), 2), (B.FitDesc(2048, 8, 0, 1e-3, B.SCD_BF16, B.SCD_F32), 3),
+                         (B.FitDesc(64, 0, 0, 1e-3, B.SCD_BF16, B.SCD_F32), 2), (B.FitDesc(64, 8, 0, 1e-3, B.SCD_F32, B.SCD_F32), 3),
+                         (B.FitDesc(64, 8, 0, 1e-3, B.SCD_BF16, B.SCD_E4M3_ROWSCALE), 1)):
+        with pytest.raises(B.ScdError) as e:
+            B.scd_fit_query(desc, 64)
+        assert e.value.status == status
+    with pytest.raises(B.ScdError):
+        B.scd_fit_query(d, 0)
