@@ -453,3 +453,15 @@ def test_paged_producer_source(name, cuda_device):
         assert torch.equal(prob.codes[b:e], want[b:e]), "codes gathered through the producer's page table differ"
     assert prob.guard_violations() == (0, 0)
     P.check_encode(prob, k, v, h)
+
+
+@pytest.mark.parametrize("rank", [64, 192, 256])
+def test_e4m3_decode_with_several_tiles_per_cta(rank, cuda_device):
+    """e4m3 codes keep the code tile of an (m-tile, segment) resident across its four n-tiles.  The mini configs give every CTA at
+    most one tile; here 21 m-tiles x 6 segments x 4 n-tiles = 504 tiles on 148 CTAs, so CTAs walk several tiles, enter and leave
+    (m-tile, segment) groups in the middle, and reuse a widened tile -- with ragged requests and permuted pages."""
+    cfg = MINI["mistral_7b_32k_fp8"].scaled(n_layers=4, patch_layers=(3,), seqlens=(1500, 1100, 7), d_model=512, rank=rank,
+                                            permute_pages=True)
+    prob = _problem(cfg, cuda_device, pos_offset=[0, 40, 3])
+    res = _run_all(prob)
+    print(rank, res)
