@@ -465,3 +465,13 @@ def test_e4m3_decode_with_several_tiles_per_cta(rank, cuda_device):
     prob = _problem(cfg, cuda_device, pos_offset=[0, 40, 3])
     res = _run_all(prob)
     print(rank, res)
+
+
+def test_patch_gemms_on_cta_pairs_with_several_tiles_per_pair(cuda_device):
+    """PATCH GEMM-2 / GEMM-3 run as CTA pairs (tcgen05 cta_group::2).  39 m-tiles (odd: the last pair has an out-of-range
+    partner) x 4 n-tiles x 2 layers = 160 / 320 pair tiles on 74 pairs: every pair walks several tiles, through the L2
+    super-block order and both accumulator buffers."""
+    cfg = MINI["llama3_8b_8k"].scaled(n_layers=2, patch_layers=(0, 1), seqlens=(3000, 1990), d_model=1024)
+    prob = _problem(cfg, cuda_device)
+    res = _run_all(prob)
+    print(res)
