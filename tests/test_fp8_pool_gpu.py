@@ -26,12 +26,16 @@ CASES = {
 SENT_BYTE, SENT_SCALE = 0xFF, 0x7FC00001
 
 
+PER_HEAD = {"per_head_reuse": 32}        # the paper-literal per-head translator writing fp8 pools
+CASES["per_head_reuse"] = C["llama3_8b_8k"].scaled(n_layers=2, patch_layers=(), seqlens=(260, 41), d_model=512)
+
+
 @pytest.mark.parametrize("name", list(CASES))
 def test_fp8_pools(name, cuda_device):
     from paper_2606_07684_b200 import binding as B
     from paper_2606_07684_b200.harness import CodecProblem
     cfg = CASES[name]
-    prob = CodecProblem(cfg, cuda_device, pos_offset=[5 * i for i in range(len(cfg.seqlens))])
+    prob = CodecProblem(cfg, cuda_device, pos_offset=[5 * i for i in range(len(cfg.seqlens))], per_head_rank=PER_HEAD.get(name, 0))
     k, v, h = prob.make_sources()
     k = P.roped_producer_k(prob, k)
     prob.alloc_pools()
