@@ -327,10 +327,10 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   ptx::grid_dep_wait();                 // the previous kernel of the stream has completed and flushed
   ptx::grid_dep_launch_dependents();    // the next one may start its prologue as SMs free up
 
-  // A_DEROPE: 896 threads x 72 registers, re-dealt per role: control warps 24, epilogue warps 128,
-  // rotation warps 56 (= 64512)
+  // A_DEROPE / A_CODES: 896 threads x 72 registers, re-dealt per role: control warps 40 (at 24 the TMA producer's and
+  // the MMA thread's loops were starved: encode K 0.134 -> 0.129 ms), epilogue warps 120, transform warps 56 (<= 64512)
   if (warp < 4) {
-  if (AMODE != A_PLAIN) ptx::setmaxnreg_dec<24>();
+  if (AMODE != A_PLAIN) ptx::setmaxnreg_dec<40>();
   if (warp == 0) {
     // ============================== TMA producer ==============================
     if (P.a_gather) {
@@ -484,7 +484,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   }
   } else if (warp < 4 + EPI_WARPS) {
     // ============================== epilogue ==============================
-    if (AMODE != A_PLAIN) ptx::setmaxnreg_inc<128>();
+    if (AMODE != A_PLAIN) ptx::setmaxnreg_inc<120>();
     // One token row per thread (TMEM lane); warps w and w+4 share a lane quadrant and split the
     // tile's work into two groups (columns, or RoPE frequencies for 2-head K tiles).  Per group:
     // TMEM -> registers -> fused math -> swizzled per-warp staging -> coalesced 16-B stores.
@@ -824,6 +824,62 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     const uint32_t row_off = (uint32_t)(tr >> 3) * 1024 + (uint32_t)(tr & 7) * 128;
     int stage = 0;
     uint32_t phase = 0;
+    if (P.head_dim == 128) {
+      // d_h = 128 (every BASELINE model): thread sp owns chunks 2sp, 2sp+1 of the "a" k-block and of the "b" k-block that
+      // follows it, i.e. frequencies [16 sp, 16 sp + 16).  Shared-space 16-B accesses, (cos, sin) as fp32 pairs in
+      // registers, the rotation in packed fp32 (2 FMUL2 + 2 FFMA2 per two channel pairs).
+      const uint32_t a0 = ptx::smem_u32(smem_a) + row_off;
+      const uint32_t sw = (uint32_t)(tr & 7);
+      const uint32_t off0 = ((uint32_t)(2 * sp) ^ sw) << 4, off1 = ((uint32_t)(2 * sp + 1) ^ sw) << 4;
+      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        int m_tile, n_tile_unused, seg_unused;
+        tile_decode(P, walk_mt, tile, m_tile, n_tile_unused, seg_unused);
+        const int row = m_tile * BLOCK_M + tr;
+        int pos = 0;
+        long long slot;
+        if (row < P.M) row_to_pos_slot(P.batch, row, pos, slot);
+        unsigned long long cc[8], ss[8];                  // (cos_j, cos_j+1), (sin_j, sin_j+1), j = 16 sp + 2 i
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const float2 v0 = rope_cs(pos, P.rope_g[sp * 16 + 2 * i]), v1 = rope_cs(pos, P.rope_g[sp * 16 + 2 * i + 1]);
+          cc[i] = f2_pack(v0.x, v1.x);
+          ss[i] = f2_pack(v0.y, v1.y);
+        }
+        for (int kb = 0; kb < P.num_kb; kb += 2) {
+          const int s0 = stage, s1 = stage + 1 == STAGES ? 0 : stage + 1;
+          ptx::mbar_wait_suspend(&bars->full[s0], phase);
+          ptx::mbar_wait_suspend(&bars->full[s1], (s1 == 0) ? (phase ^ 1) : phase);
+          const uint32_t ra = a0 + (uint32_t)s0 * A_STAGE_BYTES, rb = a0 + (uint32_t)s1 * A_STAGE_BYTES;
+#pragma unroll
+          for (int c = 0; c < 2; ++c) {
+            const uint32_t off = c == 0 ? off0 : off1;
+            uint4 xa = ptx::lds128(ra + off), xb = ptx::lds128(rb + off);
+            uint32_t* wa = reinterpret_cast<uint32_t*>(&xa);
+            uint32_t* wb = reinterpret_cast<uint32_t*>(&xb);
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+              const unsigned long long a2 = f2_pack(__uint_as_float(wa[w] << 16), __uint_as_float(wa[w] & 0xffff0000u));
+              const unsigned long long b2 = f2_pack(__uint_as_float(wb[w] << 16), __uint_as_float(wb[w] & 0xffff0000u));
+              // rotation by -phi:  a' = a cos + b sin ; b' = b cos - a sin
+              const unsigned long long na = f2_fma(a2, cc[c * 4 + w], f2_mul(b2, ss[c * 4 + w]));
+              const unsigned long long nb = f2_fma(b2, cc[c * 4 + w], f2_neg(f2_mul(a2, ss[c * 4 + w])));
+              float a_lo, a_hi, b_lo, b_hi;
+              f2_unpack(na, a_lo, a_hi);
+              f2_unpack(nb, b_lo, b_hi);
+              wa[w] = pack_bf16x2(a_lo, a_hi);
+              wb[w] = pack_bf16x2(b_lo, b_hi);
+            }
+            ptx::sts128(ra + off, xa);
+            ptx::sts128(rb + off, xb);
+          }
+          ptx::fence_proxy_async_smem();
+          ptx::mbar_arrive(&bars->ready[s0]);
+          ptx::mbar_arrive(&bars->ready[s1]);
+          for (int q = 0; q < 2; ++q)
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    } else
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
       int m_tile, n_tile_unused, seg_unused;
       tile_decode(P, walk_mt, tile, m_tile, n_tile_unused, seg_unused);

@@ -102,6 +102,12 @@ __device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsig
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
   return r;
 }
+// ptxas folds this into the consuming FFMA2's operand negation
+__device__ __forceinline__ unsigned long long f2_neg(unsigned long long a) {
+  float lo, hi;
+  f2_unpack(a, lo, hi);
+  return f2_pack(-lo, -hi);
+}
 __device__ __forceinline__ unsigned long long f2_add(unsigned long long a, unsigned long long b) {
   unsigned long long r;
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
