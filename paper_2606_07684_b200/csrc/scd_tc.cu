@@ -135,6 +135,55 @@ __device__ __forceinline__ void stg_copy_out(uint32_t stg, int pitch, int row_by
   }
 }
 
+// ---- PATCH GEMM-1 (aligner in) epilogue of a whole 256-column tile: this warp's 128 columns of its 32 rows ----
+// v = acc * scale + bias (packed fp32), SiLU(x) = h + h tanh(h) with h = x / 2 (the caller passes scale / 2 and the
+// staged bias is already halved), bf16, staged row-per-thread in the warp's [32 x 256 B] swizzled buffer.
+template <bool SILU>
+__device__ __forceinline__ void act_half_tile(uint32_t t_cols, uint32_t stg, uint32_t wvec, float scale, int lane) {
+  const unsigned long long s2 = f2_pack(scale, scale);
+#pragma unroll 1
+  for (int c = 0; c < 128; c += 32) {
+    uint32_t r[32];
+    ptx::tmem_ld32(t_cols + c, r);
+    ptx::tmem_ld_wait();
+    uint32_t o[16];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+      const float4 m4 = ptx::lds_f4(wvec + (c + q * 4) * 4);
+      float v0, v1, v2, v3;
+      f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4]), __uint_as_float(r[q * 4 + 1])), s2, f2_pack(m4.x, m4.y)), v0, v1);
+      f2_unpack(f2_fma(f2_pack(__uint_as_float(r[q * 4 + 2]), __uint_as_float(r[q * 4 + 3])), s2, f2_pack(m4.z, m4.w)), v2, v3);
+      if (SILU) {
+        float t0, t1, t2, t3;
+        asm("tanh.approx.f32 %0, %1;" : "=f"(t0) : "f"(v0));
+        asm("tanh.approx.f32 %0, %1;" : "=f"(t1) : "f"(v1));
+        asm("tanh.approx.f32 %0, %1;" : "=f"(t2) : "f"(v2));
+        asm("tanh.approx.f32 %0, %1;" : "=f"(t3) : "f"(v3));
+        v0 = fmaf(v0, t0, v0); v1 = fmaf(v1, t1, v1); v2 = fmaf(v2, t2, v2); v3 = fmaf(v3, t3, v3);
+      }
+      o[q * 2] = pack_bf16x2(v0, v1);
+      o[q * 2 + 1] = pack_bf16x2(v2, v3);
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+      ptx::sts128(stg_addr(stg, 256, lane, (c >> 3) + q), make_uint4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]));
+  }
+}
+// The staged [32 x 256 B] buffer to a row-major tensor: rows are consecutive (row r at out + r * row_stride), half a
+// warp per row, one 16-B store per lane, no per-row pointers; rows >= rows_valid (the M tail) are skipped.
+__device__ __forceinline__ void rowmajor_copy_out_256(uint32_t stg, unsigned long long out, unsigned long long row_stride,
+                                                      int rows_valid, int lane) {
+  const int chunk = lane & 15, rh = lane >> 4;
+  unsigned long long p = out + (unsigned long long)rh * row_stride + (unsigned long long)chunk * 16ull;
+#pragma unroll
+  for (int it = 0; it < 16; ++it) {
+    const int r = it * 2 + rh;
+    const uint4 v = ptx::lds128(stg_addr(stg, 256, r, chunk));
+    if (r < rows_valid) ptx::stg128(p, v);
+    p += 2ull * row_stride;
+  }
+}
+
 
 // RoPE epilogue of one K tile, specialised for HALF pairing, head_dim 128, 256-column tiles (two
 // heads).  The warp pair of a lane quadrant splits the FREQUENCIES, not the columns: warp JG owns
@@ -569,8 +618,14 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       const unsigned long long row_ptr = cur.row_ptr;
 
       // this warp's copy of the tile's mean / bias slice: wvec[c] for tile column c
+      // PATCH GEMM-1 fast path (below): whole 256-column tiles of the aligner's first layer
+      const bool act_fast = EPI == EPI_ACT && split_cols && block_n == 256 && n_end == 256;
       __syncwarp();
       if (vec_smem) {
+      if (act_fast && P.act == SCD_ACT_SILU) {             // SiLU works on h = x / 2: the bias is staged halved
+        cur.m0.x *= 0.5f; cur.m0.y *= 0.5f; cur.m0.z *= 0.5f; cur.m0.w *= 0.5f;
+        cur.m1.x *= 0.5f; cur.m1.y *= 0.5f; cur.m1.z *= 0.5f; cur.m1.w *= 0.5f;
+      }
       asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(cur.m0.x), "f"(cur.m0.y),
                    "f"(cur.m0.z), "f"(cur.m0.w) : "memory");
       asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + 512 + lane * 16), "f"(cur.m1.x), "f"(cur.m1.y),
@@ -606,6 +661,21 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         if (lane == 0) release_acc(acc);
         if (grp == 0) rope_tile_h128_copy_out<0>(stg, row_ptr, lane);
         else rope_tile_h128_copy_out<1>(stg, row_ptr, lane);
+        cur = nxt;
+        continue;
+      }
+
+      if (act_fast) {
+        // ---- PATCH GEMM-1: TMEM -> scale / bias / SiLU -> bf16 -> staging, accumulator handed back, row-major copy-out ----
+        if (P.act == SCD_ACT_SILU) act_half_tile<true>(t_row + g_begin, stg, wvec + g_begin * 4, 0.5f * rs, lane);
+        else act_half_tile<false>(t_row + g_begin, stg, wvec + g_begin * 4, rs, lane);
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (lane == 0) release_acc(acc);
+        const int row0 = m_tile * BLOCK_M + ew * 32;
+        rowmajor_copy_out_256(stg, (unsigned long long)sg.out0 + ((unsigned long long)row0 * P.N + n0 + g_begin) * 2ull,
+                              (unsigned long long)P.N * 2ull, P.M - row0, lane);
+        __syncwarp();
         cur = nxt;
         continue;
       }

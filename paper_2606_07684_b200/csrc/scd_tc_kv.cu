@@ -220,6 +220,14 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
         for (int tile = s_begin; tile < s_end; ++tile, tile_next<false>(P, tc)) {
           const TcSeg& sg = P.segs[tc.seg];
           const bool grp_first = tile == s_begin || tc.n_tile == 0;
+          if (grp_first && tile + (P.n_tiles - tc.n_tile) < s_end) {
+            // the NEXT group's code tile comes from HBM and its load sits on the critical path at the group boundary (the
+            // slots free only then): pull it into L2 now, a whole group ahead
+            int nseg = tc.seg + 1, nm = tc.m_tile;
+            if (nseg == P.n_segs) { nseg = 0; ++nm; }
+            const TcSeg& ng = P.segs[nseg];
+            for (int kb = 0; kb < P.num_kb; ++kb) ptx::tma_prefetch_l2_3d(&P.a_maps[ng.a_map], kb * BLOCK_K, nm * BLOCK_M, ng.a_z);
+          }
           for (int kb = 0; kb < P.num_kb; ++kb) {
             if (grp_first) {                                   // the code tile's k-block, once its slot has been released
               if (groups > 0) ptx::mbar_wait_suspend(&bars->a_empty[kb], (groups - 1) & 1);
