@@ -45,7 +45,13 @@ struct __align__(8) TcBarriers {
 // Shared memory is what buys pipeline stages, and three 48 KB stages (128 x 256 tiles) do not cover the TMA latency of the
 // PATCH GEMM-2 (K = d_a).  Its epilogue is off the critical path, so it stages 64 columns at a time (4 KB per warp) and reads
 // the bias straight from L1/L2 instead of a per-warp shared copy: that is the room for a fourth stage.
-static int tc_sub_n(int epi, bool compact) { return (epi == EPI_U || compact) ? 64 : SUB_N; }
+static int tc_sub_n(int epi, bool compact) { return (epi == EPI_U || epi == EPI_ACT || compact) ? 64 : SUB_N; }
+// epilogue warps of an instantiation: PATCH GEMM-1 (two k-blocks per tile, SiLU on the MUFU pipe) is paced by its epilogue,
+// so its plain-A kernel runs sixteen (four per TMEM lane quadrant, 64 columns each) -- one warp's MUFU phase overlaps the
+// others' TMEM reads and copy-out; every other kernel eight (two per quadrant)
+__host__ __device__ constexpr int tc_epi_warps(int epi, int amode, bool pair) {
+  return (epi == EPI_ACT && amode == A_PLAIN && !pair) ? 16 : EPI_WARPS;
+}
 static int tc_vec_warp_bytes(int epi, bool compact) { return (epi == EPI_U || epi == EPI_CODES || compact) ? 0 : VEC_WARP_BYTES; }
 static int tc_stg_warp_bytes(int epi, int block_n, bool compact, int out_eb) {
   if (compact) return 32 * 128;
@@ -55,12 +61,12 @@ static int tc_stg_warp_bytes(int epi, int block_n, bool compact, int out_eb) {
   return 32 * ((sub * out_eb + 127) & ~127);       // out_eb: 1 for e4m3 codes, else 2
 }
 // b_rows: rows of the B tile a CTA holds per stage (block_n, or half of it when a CTA pair shares the tile)
-static size_t tc_smem_bytes(int b_rows, int stages, int stg_warp_bytes, int vec_warp_bytes) {
+static size_t tc_smem_bytes(int b_rows, int stages, int stg_warp_bytes, int vec_warp_bytes, int epi_warps) {
   return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)b_rows * BLOCK_K * 2) +
-         EPI_WARPS * (stg_warp_bytes + vec_warp_bytes) + sizeof(TcBarriers);
+         epi_warps * (stg_warp_bytes + vec_warp_bytes) + sizeof(TcBarriers);
 }
-static int tc_pick_stages(int b_rows, int num_kb, int stg_warp_bytes, int vec_warp_bytes) {
-  const size_t budget = 232448 - 1024 - EPI_WARPS * (stg_warp_bytes + vec_warp_bytes) - sizeof(TcBarriers);
+static int tc_pick_stages(int b_rows, int num_kb, int stg_warp_bytes, int vec_warp_bytes, int epi_warps) {
+  const size_t budget = 232448 - 1024 - epi_warps * (stg_warp_bytes + vec_warp_bytes) - sizeof(TcBarriers);
   int st = (int)(budget / (A_STAGE_BYTES + (size_t)b_rows * BLOCK_K * 2));
   st = st > MAX_STAGES ? MAX_STAGES : st;
   if (st > 2 * num_kb && num_kb >= 1) st = 2 * num_kb > 2 ? 2 * num_kb : 2;   // two tiles in flight is plenty (3, 4 measured: same)
@@ -135,14 +141,14 @@ __device__ __forceinline__ void stg_copy_out(uint32_t stg, int pitch, int row_by
   }
 }
 
-// ---- PATCH GEMM-1 (aligner in) epilogue of a whole 256-column tile: this warp's 128 columns of its 32 rows ----
+// ---- PATCH GEMM-1 (aligner in) epilogue of a whole 256-column tile: 64 of this warp's columns of its 32 rows ----
 // v = acc * scale + bias (packed fp32), SiLU(x) = h + h tanh(h) with h = x / 2 (the caller passes scale / 2 and the
-// staged bias is already halved), bf16, staged row-per-thread in the warp's [32 x 256 B] swizzled buffer.
+// staged bias is already halved), bf16, staged row-per-thread in the warp's [32 x 128 B] swizzled buffer.
 template <bool SILU>
-__device__ __forceinline__ void act_half_tile(uint32_t t_cols, uint32_t stg, uint32_t wvec, float scale, int lane) {
+__device__ __forceinline__ void act_stage64(uint32_t t_cols, uint32_t stg, uint32_t wvec, float scale, int lane) {
   const unsigned long long s2 = f2_pack(scale, scale);
 #pragma unroll 1
-  for (int c = 0; c < 128; c += 32) {
+  for (int c = 0; c < 64; c += 32) {
     uint32_t r[32];
     ptx::tmem_ld32(t_cols + c, r);
     ptx::tmem_ld_wait();
@@ -166,24 +172,23 @@ __device__ __forceinline__ void act_half_tile(uint32_t t_cols, uint32_t stg, uin
     }
 #pragma unroll
     for (int q = 0; q < 4; ++q)
-      ptx::sts128(stg_addr(stg, 256, lane, (c >> 3) + q), make_uint4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]));
+      ptx::sts128(stg_addr(stg, 128, lane, (c >> 3) + q), make_uint4(o[4 * q], o[4 * q + 1], o[4 * q + 2], o[4 * q + 3]));
   }
 }
-// The staged [32 x 256 B] buffer to a row-major tensor: rows are consecutive (row r at out + r * row_stride), half a
-// warp per row, one 16-B store per lane, no per-row pointers; rows >= rows_valid (the M tail) are skipped.
-__device__ __forceinline__ void rowmajor_copy_out_256(uint32_t stg, unsigned long long out, unsigned long long row_stride,
+// The staged [32 x 128 B] buffer to a row-major tensor: rows are consecutive (row r at out + r * row_stride), eight lanes
+// per row, one 16-B store per lane, no per-row pointers; rows >= rows_valid (the M tail) are skipped.
+__device__ __forceinline__ void rowmajor_copy_out_128(uint32_t stg, unsigned long long out, unsigned long long row_stride,
                                                       int rows_valid, int lane) {
-  const int chunk = lane & 15, rh = lane >> 4;
-  unsigned long long p = out + (unsigned long long)rh * row_stride + (unsigned long long)chunk * 16ull;
+  const int chunk = lane & 7, rq = lane >> 3;
+  unsigned long long p = out + (unsigned long long)rq * row_stride + (unsigned long long)chunk * 16ull;
 #pragma unroll
-  for (int it = 0; it < 16; ++it) {
-    const int r = it * 2 + rh;
-    const uint4 v = ptx::lds128(stg_addr(stg, 256, r, chunk));
+  for (int it = 0; it < 8; ++it) {
+    const int r = it * 4 + rq;
+    const uint4 v = ptx::lds128(stg_addr(stg, 128, r, chunk));
     if (r < rows_valid) ptx::stg128(p, v);
-    p += 2ull * row_stride;
+    p += 4ull * row_stride;
   }
 }
-
 
 // RoPE epilogue of one K tile, specialised for HALF pairing, head_dim 128, 256-column tiles (two
 // heads).  The warp pair of a lane quadrant splits the FREQUENCIES, not the columns: warp JG owns
@@ -324,9 +329,10 @@ __device__ __forceinline__ void rope_tile_h128_copy_out(uint32_t stg, unsigned l
 // barriers, its commits are multicast to both CTAs' `empty` / `tmem_full` barriers, and the epilogue warps of both CTAs
 // hand accumulators back on its `tmem_empty` barriers.  Tile = (segment, n-tile, pair of m-tiles).
 template <int EPI, int AMODE, bool PAIR = false>
-__global__ void __launch_bounds__(AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, 1)
+__global__ void __launch_bounds__(AMODE != A_PLAIN ? DEROPE_NTHREADS : (4 + tc_epi_warps(EPI, AMODE, PAIR)) * 32, 1)
 tc_gemm_kernel(const __grid_constant__ TcParams P) {
   static_assert(!PAIR || AMODE == A_PLAIN, "CTA pairs: plain A operands only");
+  constexpr int NEPI = tc_epi_warps(EPI, AMODE, PAIR);           // epilogue warps: 8, or 16 for PATCH GEMM-1
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int block_n = P.block_n;
@@ -339,10 +345,10 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
   uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
-  uint8_t* smem_vec = smem_stg + EPI_WARPS * P.stg_warp_bytes;
+  uint8_t* smem_vec = smem_stg + NEPI * P.stg_warp_bytes;
   constexpr bool VEC_SMEM = (EPI == EPI_KV || EPI == EPI_ACT);   // else the mean / bias is read through L1 (tc_vec_warp_bytes)
   const bool vec_smem = VEC_SMEM && !(EPI == EPI_KV && P.kv_compact);
-  TcBarriers* bars = (TcBarriers*)(smem_vec + (vec_smem ? EPI_WARPS * VEC_WARP_BYTES : 0));
+  TcBarriers* bars = (TcBarriers*)(smem_vec + (vec_smem ? NEPI * VEC_WARP_BYTES : 0));
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.n_segs * P.n_tiles * walk_mt;
@@ -355,7 +361,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
-      ptx::mbar_init(&bars->tmem_empty[a], PAIR ? 2 * EPI_WARPS : EPI_WARPS);
+      ptx::mbar_init(&bars->tmem_empty[a], PAIR ? 2 * EPI_WARPS : NEPI);
     }
     ptx::fence_barrier_init();
   }
@@ -531,7 +537,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       }
     }
   }
-  } else if (warp < 4 + EPI_WARPS) {
+  } else if (warp < 4 + NEPI) {
     // ============================== epilogue ==============================
     if (AMODE != A_PLAIN) ptx::setmaxnreg_inc<120>();
     // One token row per thread (TMEM lane); warps w and w+4 share a lane quadrant and split the
@@ -619,7 +625,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // this warp's copy of the tile's mean / bias slice: wvec[c] for tile column c
       // PATCH GEMM-1 fast path (below): whole 256-column tiles of the aligner's first layer
-      const bool act_fast = EPI == EPI_ACT && split_cols && block_n == 256 && n_end == 256;
+      const bool act_fast = EPI == EPI_ACT && block_n == 256 && n_end == 256;
       __syncwarp();
       if (vec_smem) {
       if (act_fast && P.act == SCD_ACT_SILU) {             // SiLU works on h = x / 2: the bias is staged halved
@@ -667,15 +673,21 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       if (act_fast) {
         // ---- PATCH GEMM-1: TMEM -> scale / bias / SiLU -> bf16 -> staging, accumulator handed back, row-major copy-out ----
-        if (P.act == SCD_ACT_SILU) act_half_tile<true>(t_row + g_begin, stg, wvec + g_begin * 4, 0.5f * rs, lane);
-        else act_half_tile<false>(t_row + g_begin, stg, wvec + g_begin * 4, rs, lane);
-        ptx::tc_fence_before();
-        __syncwarp();
-        if (lane == 0) release_acc(acc);
+        // warp (quadrant ew, group grp) owns columns [grp * cw, (grp + 1) * cw), cw = 64 (sixteen warps) or 128 (eight)
+        constexpr int CW = 256 / (NEPI / 4), PASSES = CW / 64;
         const int row0 = m_tile * BLOCK_M + ew * 32;
-        rowmajor_copy_out_256(stg, (unsigned long long)sg.out0 + ((unsigned long long)row0 * P.N + n0 + g_begin) * 2ull,
-                              (unsigned long long)P.N * 2ull, P.M - row0, lane);
-        __syncwarp();
+        const unsigned long long out_q = (unsigned long long)sg.out0 + ((unsigned long long)row0 * P.N + n0 + grp * CW) * 2ull;
+#pragma unroll
+        for (int ps = 0; ps < PASSES; ++ps) {
+          const int c0 = grp * CW + ps * 64;
+          if (P.act == SCD_ACT_SILU) act_stage64<true>(t_row + c0, stg, wvec + c0 * 4, 0.5f * rs, lane);
+          else act_stage64<false>(t_row + c0, stg, wvec + c0 * 4, rs, lane);
+          if (ps == PASSES - 1) ptx::tc_fence_before();
+          __syncwarp();
+          if (ps == PASSES - 1 && lane == 0) release_acc(acc);
+          rowmajor_copy_out_128(stg, out_q + (unsigned long long)ps * 128ull, (unsigned long long)P.N * 2ull, P.M - row0, lane);
+          __syncwarp();
+        }
         cur = nxt;
         continue;
       }
@@ -1237,7 +1249,8 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
                      (EPI == EPI_CODES && (P.block_n % 32) == 0));
   if (P.pair && !pair) return fail(SCD_E_UNSUPPORTED, "internal: CTA-pair launch requested for a shape it does not take");
   const int b_rows = pair ? P.block_n / 2 : P.block_n;
-  P.stages = tc_pick_stages(b_rows, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
+  constexpr int NEPI = tc_epi_warps(EPI, AMODE, false);
+  P.stages = tc_pick_stages(b_rows, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), pair ? EPI_WARPS : NEPI);
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
   P.a_prefetch = (EPI == EPI_CODES && !P.a_gather) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
   const int walk_mt = pair ? (P.m_tiles + 1) / 2 : P.m_tiles;      // m-tiles of the walk (pair tiles of 256 rows)
@@ -1247,7 +1260,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
     int msb = (int)std::max<long long>(1, (32ll << 20) / a_tile_bytes);
     if (msb < walk_mt) P.msb = msb;
   }
-  const size_t smem = tc_smem_bytes(b_rows, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact));
+  const size_t smem = tc_smem_bytes(b_rows, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), pair ? EPI_WARPS : NEPI);
   if (pair) return launch_tc_pair<EPI>(p, P, smem, P.n_segs * P.n_tiles * walk_mt, s);
   // the attribute belongs to (function, device): cached per instantiation and device ordinal
   static std::atomic<size_t> configured[SCD_MAX_DEVICES];
@@ -1258,7 +1271,7 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   }
   const int grid = std::min(total, p->sm_count);
   prof_begin(s);
-  launch_pdl(tc_gemm_kernel<EPI, AMODE>, grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : 384, smem, s, 1, P);
+  launch_pdl(tc_gemm_kernel<EPI, AMODE>, grid, AMODE != A_PLAIN ? DEROPE_NTHREADS : (4 + NEPI) * 32, smem, s, 1, P);
   prof_end(s, P.prof_id);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_gemm_kernel launch: %s", cudaGetErrorString(e));
