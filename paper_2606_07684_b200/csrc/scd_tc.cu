@@ -37,6 +37,7 @@ constexpr int DEROPE_NTHREADS = (4 + EPI_WARPS + DEROPE_WARPS) * 32;   // 896
 struct __align__(8) TcBarriers {
   uint64_t full[MAX_STAGES], empty[MAX_STAGES], ready[MAX_STAGES];
   uint64_t tmem_full[2], tmem_empty[2];
+  uint64_t b_full[4], b_empty[4];              // B-resident mode (PATCH GEMM-1): the resident B tile's k-block slots
   uint32_t tmem_base;
 };
 
@@ -64,6 +65,17 @@ static int tc_stg_warp_bytes(int epi, int block_n, bool compact, int out_eb) {
 static size_t tc_smem_bytes(int b_rows, int stages, int stg_warp_bytes, int vec_warp_bytes, int epi_warps) {
   return 1024 /*align slack*/ + (size_t)stages * (A_STAGE_BYTES + (size_t)b_rows * BLOCK_K * 2) +
          epi_warps * (stg_warp_bytes + vec_warp_bytes) + sizeof(TcBarriers);
+}
+// B-resident mode: num_kb slots for the B tile + a ring of A stages
+static size_t tc_smem_bytes_bres(int b_rows, int num_kb, int stages, int stg_warp_bytes, int vec_warp_bytes, int epi_warps) {
+  return 1024 + (size_t)stages * A_STAGE_BYTES + (size_t)num_kb * b_rows * BLOCK_K * 2 + epi_warps * (stg_warp_bytes + vec_warp_bytes) +
+         sizeof(TcBarriers);
+}
+static int tc_pick_stages_bres(int b_rows, int num_kb, int stg_warp_bytes, int vec_warp_bytes, int epi_warps) {
+  const long long budget = 232448 - 1024 - epi_warps * (stg_warp_bytes + vec_warp_bytes) - (long long)sizeof(TcBarriers) -
+                           (long long)num_kb * b_rows * BLOCK_K * 2;
+  const int st = (int)(budget / A_STAGE_BYTES);
+  return st > MAX_STAGES ? MAX_STAGES : st;
 }
 static int tc_pick_stages(int b_rows, int num_kb, int stg_warp_bytes, int vec_warp_bytes, int epi_warps) {
   const size_t budget = 232448 - 1024 - epi_warps * (stg_warp_bytes + vec_warp_bytes) - sizeof(TcBarriers);
@@ -342,9 +354,14 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   const int walker = PAIR ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;            // index of this CTA (pair) in the tile walk
   const int walk_stride = PAIR ? (int)(gridDim.x >> 1) : (int)gridDim.x;
   const int STAGES = P.stages;
+  // B-resident mode (PATCH GEMM-1: K = r_h is one or two k-blocks, so the 64 KB B tile is two thirds of a tile's operand bytes):
+  // each CTA walks a CONTIGUOUS share of the (segment, n-tile, m-tile) order, m fastest, keeps the B tile of its (segment,
+  // n-tile) in slots of its own and streams only the A tiles through the ring
+  constexpr bool BRES_OK = EPI == EPI_ACT && AMODE == A_PLAIN && !PAIR;
+  const bool bres = BRES_OK && P.b_res;
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + STAGES * A_STAGE_BYTES;
-  uint8_t* smem_stg = smem_b + STAGES * b_stage_bytes;
+  uint8_t* smem_stg = smem_b + (bres ? P.num_kb : STAGES) * b_stage_bytes;
   uint8_t* smem_vec = smem_stg + NEPI * P.stg_warp_bytes;
   constexpr bool VEC_SMEM = (EPI == EPI_KV || EPI == EPI_ACT);   // else the mean / bias is read through L1 (tc_vec_warp_bytes)
   const bool vec_smem = VEC_SMEM && !(EPI == EPI_KV && P.kv_compact);
@@ -352,12 +369,20 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.n_segs * P.n_tiles * walk_mt;
+  // this CTA's tiles: t_begin, t_begin + t_step, ... < t_end
+  const int t_begin = bres ? (int)((long long)blockIdx.x * total_tiles / gridDim.x) : walker;
+  const int t_end = bres ? (int)((long long)(blockIdx.x + 1) * total_tiles / gridDim.x) : total_tiles;
+  const int t_step = bres ? 1 : walk_stride;
 
   if (warp == 0 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
       ptx::mbar_init(&bars->full[s], 1);
       ptx::mbar_init(&bars->empty[s], 1);
       ptx::mbar_init(&bars->ready[s], DEROPE_WARPS * 32);
+    }
+    for (int k = 0; k < 4; ++k) {
+      ptx::mbar_init(&bars->b_full[k], 1);
+      ptx::mbar_init(&bars->b_empty[k], 1);
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
@@ -459,6 +484,31 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
           }
         }
       }
+    } else if (bres) {
+      if (lane == 0) {
+        int stage = 0, prev_key = -1;
+        uint32_t phase = 0, groups = 0;                         // groups = (segment, n-tile) B tiles started so far
+        for (int tile = t_begin; tile < t_end; ++tile) {
+          int m_tile, n_tile, seg_i;
+          tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
+          const TcSeg& sg = P.segs[seg_i];
+          const int key = seg_i * P.n_tiles + n_tile;
+          const bool grp_first = key != prev_key;
+          prev_key = key;
+          for (int kb = 0; kb < P.num_kb; ++kb) {
+            if (grp_first) {                                     // the B tile's k-block, once the previous group's MMAs are done with the slot
+              if (groups > 0) ptx::mbar_wait_suspend(&bars->b_empty[kb], (groups - 1) & 1);
+              ptx::mbar_expect_tx(&bars->b_full[kb], b_stage_bytes);
+              ptx::tma_load_2d(smem_b + kb * b_stage_bytes, P.b_maps + sg.b_map, &bars->b_full[kb], kb * BLOCK_K, n_tile * block_n);
+            }
+            ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
+            ptx::mbar_expect_tx(&bars->full[stage], A_STAGE_BYTES);
+            ptx::tma_load_3d(smem_a + stage * A_STAGE_BYTES, &P.a_maps[sg.a_map], &bars->full[stage], kb * BLOCK_K, m_tile * BLOCK_M, sg.a_z);
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+          if (grp_first) ++groups;
+        }
+      }
     } else
     if (lane == 0) {
       int stage = 0;
@@ -507,6 +557,45 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     }
   } else if (warp == 1) {
     // ============================== MMA issuer ==============================
+    if (bres) {
+      if (lane == 0) {
+        const uint32_t idesc = ptx::umma_idesc_bf16(BLOCK_M, block_n);
+        int stage = 0, it = 0;
+        uint32_t phase = 0, groups = 0;                         // groups completed
+        int m_tile, n_tile, seg_i;
+        if (t_begin < t_end) tile_decode(P, walk_mt, t_begin, m_tile, n_tile, seg_i);
+        int key = t_begin < t_end ? seg_i * P.n_tiles + n_tile : -1, prev_key = -1;
+        for (int tile = t_begin; tile < t_end; ++tile, ++it) {
+          int next_key = -1;
+          if (tile + 1 < t_end) {
+            tile_decode(P, walk_mt, tile + 1, m_tile, n_tile, seg_i);
+            next_key = seg_i * P.n_tiles + n_tile;
+          }
+          const bool grp_first = key != prev_key, grp_last = next_key != key;
+          const int acc = it & 1;
+          ptx::mbar_wait_suspend(&bars->tmem_empty[acc], ((it >> 1) & 1) ^ 1);
+          ptx::tc_fence_after();
+          const uint32_t d_tmem = tmem_base + (uint32_t)(acc * 256);
+          for (int kb = 0; kb < P.num_kb; ++kb) {
+            if (grp_first) ptx::mbar_wait_suspend(&bars->b_full[kb], groups & 1);
+            ptx::mbar_wait_suspend(&bars->full[stage], phase);
+            ptx::tc_fence_after();
+            const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + stage * A_STAGE_BYTES));
+            const uint64_t db = ptx::umma_desc_sw128(ptx::smem_u32(smem_b + kb * b_stage_bytes));
+#pragma unroll
+            for (int k = 0; k < BLOCK_K / 16; ++k)
+              ptx::mma_bf16(d_tmem, da + (uint64_t)(k * 2), db + (uint64_t)(k * 2), idesc, (kb | k) != 0);
+            ptx::mma_commit(&bars->empty[stage]);
+            if (grp_last) ptx::mma_commit(&bars->b_empty[kb]);   // the slot may take the next group's B tile
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+          ptx::mma_commit(&bars->tmem_full[acc]);
+          if (grp_last) ++groups;
+          prev_key = key;
+          key = next_key;
+        }
+      }
+    } else
     if (lane == 0 && cta_rank == 0) {
       const uint32_t idesc = ptx::umma_idesc_bf16(PAIR ? 2 * BLOCK_M : BLOCK_M, block_n);
       int stage = 0;
@@ -602,10 +691,54 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       if (PAIR) ptx::mbar_arrive_cluster(ptx::mapa(ptx::smem_u32(&bars->tmem_empty[acc]), 0));
       else ptx::mbar_arrive(&bars->tmem_empty[acc]);
     };
+    if (bres) {
+      // ---- PATCH GEMM-1, B-resident walk: consecutive tiles are consecutive m-tiles of one (segment, n-tile), so the tile
+      // coordinates advance without divisions and the warp's 64-entry bias slice is staged once per (segment, n-tile) ----
+      constexpr int CW = 256 / (NEPI / 4), PASSES = CW / 64;
+      int m_tile = 0, n_tile = 0, seg_i = 0, prev_key = -1;
+      if (t_begin < t_end) tile_decode(P, walk_mt, t_begin, m_tile, n_tile, seg_i);
+      const bool silu = P.act == SCD_ACT_SILU;
+      int it = 0;
+      for (int tile = t_begin; tile < t_end; ++tile, ++it) {
+        const TcSeg& sg = P.segs[seg_i];
+        const int n0 = n_tile * block_n;
+        const int key = seg_i * P.n_tiles + n_tile;
+        if (key != prev_key) {
+          prev_key = key;
+          __syncwarp();
+          for (int i = lane; i < CW / 4; i += 32) {
+            float4 b4 = sg.col_vec ? ldg_f4(sg.col_vec + n0 + grp * CW + i * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+            if (silu) { b4.x *= 0.5f; b4.y *= 0.5f; b4.z *= 0.5f; b4.w *= 0.5f; }   // SiLU works on h = x / 2
+            asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + i * 16), "f"(b4.x), "f"(b4.y), "f"(b4.z), "f"(b4.w) : "memory");
+          }
+          __syncwarp();
+        }
+        const int acc = it & 1;
+        ptx::mbar_wait_suspend(&bars->tmem_full[acc], (it >> 1) & 1);
+        ptx::tc_fence_after();
+        const uint32_t t_row = tmem_base + (uint32_t)(acc * 256) + ((uint32_t)(ew * 32) << 16);
+        const int row0 = m_tile * BLOCK_M + ew * 32;
+        const unsigned long long out_q = (unsigned long long)sg.out0 + ((unsigned long long)row0 * P.N + n0 + grp * CW) * 2ull;
+#pragma unroll
+        for (int ps = 0; ps < PASSES; ++ps) {
+          if (silu) act_stage64<true>(t_row + grp * CW + ps * 64, stg, wvec + ps * 256, 0.5f, lane);
+          else act_stage64<false>(t_row + grp * CW + ps * 64, stg, wvec + ps * 256, 1.0f, lane);
+          if (ps == PASSES - 1) ptx::tc_fence_before();
+          __syncwarp();
+          if (ps == PASSES - 1 && lane == 0) release_acc(acc);
+          rowmajor_copy_out_128(stg, out_q + (unsigned long long)ps * 128ull, (unsigned long long)P.N * 2ull, P.M - row0, lane);
+          __syncwarp();
+        }
+        if (++m_tile == walk_mt) {                              // plain m-fastest order (the host checks msb >= m-tiles)
+          m_tile = 0;
+          if (++n_tile == P.n_tiles) { n_tile = 0; ++seg_i; }
+        }
+      }
+    } else {
     int it = 0;
     RowInfo cur;
-    if (walker < total_tiles) cur = fetch(walker);
-    for (int tile = walker; tile < total_tiles; tile += walk_stride, ++it) {
+    if (t_begin < t_end) cur = fetch(t_begin);
+    for (int tile = t_begin; tile < t_end; tile += t_step, ++it) {
       int m_tile, n_tile, seg_i;
       tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
       if (PAIR) m_tile = 2 * m_tile + (int)cta_rank;
@@ -645,7 +778,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // prefetch the next tile's per-row quantities; consumed at the bottom of the loop
       RowInfo nxt = cur;
-      if (tile + walk_stride < total_tiles) nxt = fetch(tile + walk_stride);
+      if (tile + t_step < t_end) nxt = fetch(tile + t_step);
 
       if (EPI == EPI_KV && n0 < sg.rope_cols && P.rope_style == SCD_ROPE_HALF && P.head_dim == 128 && block_n == 256 &&
           n_end == 256) {
@@ -846,6 +979,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       }
       if (EPI == EPI_U && valid && sg.aux) sg.aux[(size_t)(n_tile * 2 + grp) * P.M + row] = ss_u;
       cur = nxt;
+    }
     }
   } else if (AMODE == A_CODES) {
     // ============================== A transform: e4m3 -> bf16 in shared memory ==============================
@@ -1131,6 +1265,9 @@ static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, i
 #ifndef TC_ENC_PAIRS
 #define TC_ENC_PAIRS 1
 #endif
+#ifndef TC_G1_BRES
+#define TC_G1_BRES 1
+#endif
 #ifndef TC_A_PREFETCH
 #define TC_A_PREFETCH 4
 #endif
@@ -1251,6 +1388,14 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
   const int b_rows = pair ? P.block_n / 2 : P.block_n;
   constexpr int NEPI = tc_epi_warps(EPI, AMODE, false);
   P.stages = tc_pick_stages(b_rows, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), pair ? EPI_WARPS : NEPI);
+  // PATCH GEMM-1 with short K: B tile resident, A tiles streamed (see the kernel); needs a few tiles per CTA to pay
+  const bool bres = TC_G1_BRES && EPI == EPI_ACT && AMODE == A_PLAIN && !pair && P.num_kb <= 4 && P.a_kb_per_head == 0 &&
+                    total >= 4 * p->sm_count && P.block_n == 256 && (P.N % 256) == 0 &&
+                    tc_pick_stages_bres(b_rows, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), NEPI) >= 2 * P.num_kb;
+  if (bres) {
+    P.b_res = 1;
+    P.stages = tc_pick_stages_bres(b_rows, P.num_kb, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), NEPI);
+  }
   // super-block so that its A rows take <= 32 MB of the 126 MB L2 (whole CTA waves: a multiple of the grid's share)
   P.a_prefetch = (EPI == EPI_CODES && !P.a_gather) ? TC_A_PREFETCH : 0;   // encode: A is the HBM stream
   const int walk_mt = pair ? (P.m_tiles + 1) / 2 : P.m_tiles;      // m-tiles of the walk (pair tiles of 256 rows)
@@ -1260,7 +1405,9 @@ static scd_status_t launch_tc(const scd_plan_t* p, TcParams& P, cudaStream_t s) 
     int msb = (int)std::max<long long>(1, (32ll << 20) / a_tile_bytes);
     if (msb < walk_mt) P.msb = msb;
   }
-  const size_t smem = tc_smem_bytes(b_rows, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), pair ? EPI_WARPS : NEPI);
+  if (bres) P.msb = walk_mt;                                       // plain m-fastest order (A is K <= 256 wide: nothing to block)
+  const size_t smem = bres ? tc_smem_bytes_bres(b_rows, P.num_kb, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), NEPI)
+                           : tc_smem_bytes(b_rows, P.stages, P.stg_warp_bytes, tc_vec_warp_bytes(EPI, compact), pair ? EPI_WARPS : NEPI);
   if (pair) return launch_tc_pair<EPI>(p, P, smem, P.n_segs * P.n_tiles * walk_mt, s);
   // the attribute belongs to (function, device): cached per instantiation and device ordinal
   static std::atomic<size_t> configured[SCD_MAX_DEVICES];
