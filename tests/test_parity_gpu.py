@@ -478,3 +478,13 @@ def test_patch_gemms_on_cta_pairs_with_several_tiles_per_pair(cuda_device):
     prob = _problem(cfg, cuda_device)
     res = _run_all(prob)
     print(res)
+
+
+def test_patch_gemm1_b_resident_walk_with_a_ragged_tail(cuda_device):
+    """PATCH GEMM-1 with enough tiles for the B-resident walk (4 layers x 4 n-tiles x 39 m-tiles = 624 >= 4 x 148): every CTA
+    owns a contiguous run of ~4 m-tiles, runs cross (layer, n-tile) boundaries -- the resident W1 tile is swapped mid-run, the
+    staged bias slice with it -- and the last m-tile has 126 valid rows.  All layers are PATCH layers."""
+    cfg = MINI["llama3_8b_8k"].scaled(n_layers=4, patch_layers=(0, 1, 2, 3), seqlens=(3000, 1990), d_model=1024)
+    prob = _problem(cfg, cuda_device)
+    res = _run_all(prob)
+    print(res)
