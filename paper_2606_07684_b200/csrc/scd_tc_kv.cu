@@ -556,22 +556,23 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
       if (tile + 1 < t_end) nxt = fetch(tn);
 
       if (is_k) {
-        // ---- K tile: rotate pairs (j, j + 64) of both heads, j in [16g, 16g + 16) ----
+        // ---- K tile: rotate pairs (j, j + 64) of both heads, j in [16g, 16g + 16), eight pairs at a time ----
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          uint32_t ra[16], rb[16];
-          const int ca = h * 128 + 16 * g;
-          ptx::tmem_ld16(t_row + ca, ra);
-          ptx::tmem_ld16(t_row + ca + 64, rb);
+        for (int hh = 0; hh < 4; ++hh) {
+          const int h = hh >> 1, hf = hh & 1;                   // head of the tile, half of the warp's 16 frequencies
+          uint32_t ra[8], rb[8];
+          const int ca = h * 128 + 16 * g + 8 * hf;
+          ptx::tmem_ld8(t_row + ca, ra);
+          ptx::tmem_ld8(t_row + ca + 64, rb);
           ptx::tmem_ld_wait();
-          uint32_t oa[8], ob[8];
+          uint32_t oa[4], ob[4];
 #pragma unroll
-          for (int q4 = 0; q4 < 4; ++q4) {
-            const float4 ma = ptx::lds_f4(wvec + ((2 * h) * 16 + q4 * 4) * 4);
-            const float4 mb = ptx::lds_f4(wvec + ((2 * h + 1) * 16 + q4 * 4) * 4);
+          for (int q4 = 0; q4 < 2; ++q4) {
+            const float4 ma = ptx::lds_f4(wvec + ((2 * h) * 16 + 8 * hf + q4 * 4) * 4);
+            const float4 mb = ptx::lds_f4(wvec + ((2 * h + 1) * 16 + 8 * hf + q4 * 4) * 4);
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
-              const int i = q4 * 4 + e * 2, k = q4 * 2 + e;
+              const int i = q4 * 4 + e * 2, k = q4 * 2 + e, kf = 4 * hf + k;
               const unsigned long long am = e ? f2_pack(ma.z, ma.w) : f2_pack(ma.x, ma.y);
               const unsigned long long bm = e ? f2_pack(mb.z, mb.w) : f2_pack(mb.x, mb.y);
               const unsigned long long av = f2_pack(__uint_as_float(ra[i]), __uint_as_float(ra[i + 1]));
@@ -579,31 +580,30 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
               const unsigned long long a = SCALED ? f2_fma(av, rs2, am) : f2_add(av, am);
               const unsigned long long b = SCALED ? f2_fma(bv, rs2, bm) : f2_add(bv, bm);
               float x0, x1, y0, y1, t0, t1;
-              f2_unpack(f2_mul(b, s2[k]), t0, t1);
-              f2_unpack(f2_fma(a, c2[k], f2_pack(-t0, -t1)), x0, x1);     // a cos - b sin
-              f2_unpack(f2_fma(a, s2[k], f2_mul(b, c2[k])), y0, y1);      // b cos + a sin
+              f2_unpack(f2_mul(b, s2[kf]), t0, t1);
+              f2_unpack(f2_fma(a, c2[kf], f2_pack(-t0, -t1)), x0, x1);    // a cos - b sin
+              f2_unpack(f2_fma(a, s2[kf], f2_mul(b, c2[kf])), y0, y1);    // b cos + a sin
               oa[k] = pack_bf16x2(x0, x1);
               ob[k] = pack_bf16x2(y0, y1);
             }
           }
-          if (h == 0) ptx::named_bar_sync(bar_id, 128);         // the quadrant's previous copy-out has drained
-          const int k0 = h * 16 + 2 * g;                        // 16-B chunk of run (h, a); run (h, b) = +8
+          if (hh == 0) ptx::named_bar_sync(bar_id, 128);        // the quadrant's previous copy-out has drained
+          const int k0 = h * 16 + 2 * g + hf;                   // 16-B chunk of run (h, a); run (h, b) = +8
           ptx::sts128(qstg_addr(stg, lane, k0), make_uint4(oa[0], oa[1], oa[2], oa[3]));
-          ptx::sts128(qstg_addr(stg, lane, k0 + 1), make_uint4(oa[4], oa[5], oa[6], oa[7]));
           ptx::sts128(qstg_addr(stg, lane, k0 + 8), make_uint4(ob[0], ob[1], ob[2], ob[3]));
-          ptx::sts128(qstg_addr(stg, lane, k0 + 9), make_uint4(ob[4], ob[5], ob[6], ob[7]));
         }
       } else {
-        // ---- V tile (or K without RoPE): columns [64g, 64g + 64), 32 at a time ----
+        // ---- V tile (or K without RoPE): columns [64g, 64g + 64), 16 at a time (32 at a time cost 12 B of spills at the
+        // epilogue's 112-register cap, and a spill reload queues behind the copy-out stores) ----
 #pragma unroll
-        for (int c = 0; c < 2; ++c) {
-          uint32_t r[32];
-          ptx::tmem_ld32(t_row + 64 * g + 32 * c, r);
+        for (int c = 0; c < 4; ++c) {
+          uint32_t r[16];
+          ptx::tmem_ld16(t_row + 64 * g + 16 * c, r);
           ptx::tmem_ld_wait();
-          uint32_t o[16];
+          uint32_t o[8];
 #pragma unroll
-          for (int q4 = 0; q4 < 8; ++q4) {
-            const float4 m4 = ptx::lds_f4(wvec + (c * 32 + q4 * 4) * 4);
+          for (int q4 = 0; q4 < 4; ++q4) {
+            const float4 m4 = ptx::lds_f4(wvec + (c * 16 + q4 * 4) * 4);
             float v0, v1, v2, v3;
             const unsigned long long r01 = f2_pack(__uint_as_float(r[q4 * 4]), __uint_as_float(r[q4 * 4 + 1]));
             const unsigned long long r23 = f2_pack(__uint_as_float(r[q4 * 4 + 2]), __uint_as_float(r[q4 * 4 + 3]));
@@ -613,10 +613,9 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
             o[q4 * 2 + 1] = pack_bf16x2(v2, v3);
           }
           if (c == 0) ptx::named_bar_sync(bar_id, 128);
-          const int k0 = 8 * g + 4 * c;
-#pragma unroll
-          for (int j = 0; j < 4; ++j)
-            ptx::sts128(qstg_addr(stg, lane, k0 + j), make_uint4(o[4 * j], o[4 * j + 1], o[4 * j + 2], o[4 * j + 3]));
+          const int k0 = 8 * g + 2 * c;
+          ptx::sts128(qstg_addr(stg, lane, k0), make_uint4(o[0], o[1], o[2], o[3]));
+          ptx::sts128(qstg_addr(stg, lane, k0 + 1), make_uint4(o[4], o[5], o[6], o[7]));
         }
       }
       // staging complete and all TMEM reads of the quadrant done: hand the accumulator back, copy out
