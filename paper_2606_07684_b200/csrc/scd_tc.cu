@@ -404,7 +404,11 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   else __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
-  ptx::grid_dep_wait();                 // the previous kernel of the stream has completed and flushed
+  // The previous kernel of the stream has completed and flushed -- unless this launch is independent of it (P.dep_wait_late:
+  // the 2nd, 3rd ... launch of one scd_encode call reads the caller's states and writes its own code segments), in which case
+  // its CTAs start working as the predecessor's last wave frees SMs and wait for it at their END instead, so that this grid's
+  // completion still implies the predecessor's (the next call's first kernel waits on the last launch only).
+  if (!P.dep_wait_late) ptx::grid_dep_wait();
   ptx::grid_dep_launch_dependents();    // the next one may start its prologue as SMs free up
 
   // A_DEROPE / A_CODES: 896 threads x 72 registers, re-dealt per role: control warps 40 (at 24 the TMA producer's and
@@ -1153,6 +1157,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
   // ============================== teardown ==============================
   ptx::tc_fence_before();
+  if (P.dep_wait_late && threadIdx.x == 0) ptx::grid_dep_wait();
   if (PAIR) {
     ptx::cluster_sync();                // neither CTA leaves while the other may still signal its barriers / read its TMEM
     if (warp == 2) ptx::tmem_dealloc_cg2<TMEM_COLS>(tmem_base);
@@ -1264,6 +1269,9 @@ static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, i
 #endif
 #ifndef TC_ENC_PAIRS
 #define TC_ENC_PAIRS 1
+#endif
+#ifndef TC_ENC_OVERLAP
+#define TC_ENC_OVERLAP 1
 #endif
 #ifndef TC_G1_BRES
 #define TC_G1_BRES 1
@@ -1470,6 +1478,7 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
     return fail(SCD_E_UNSUPPORTED, "head-strided K/V needs head_dim %% 64 == 0");
 
   size_t i = 0;
+  int n_launched = 0;
   const size_t nseg = p->segs.size();
   while (i < nseg) {
     if (!layer_in_window(p->segs[i].layer)) { ++i; continue; }
@@ -1527,6 +1536,8 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
       if (st != SCD_OK) return st;
     }
     P.prof_id = (s0.branch == SCD_BRANCH_K && m.k_is_roped) ? SCD_PROF_ENCODE_K : SCD_PROF_ENCODE;
+    P.dep_wait_late = (TC_ENC_OVERLAP && n_launched > 0) ? 1 : 0;      // the call's launches are independent of one another
+    ++n_launched;
     if (s0.branch == SCD_BRANCH_K && m.k_is_roped) {
       if (m.rope_style != SCD_ROPE_HALF)
         return fail(SCD_E_UNSUPPORTED, "deRoPE-on-load implements the HALF pairing only on the bf16 path");
