@@ -222,6 +222,29 @@ scd_status_t scd_patch_layers(const scd_plan_t* plan, const scd_batch_t* batch, 
                               int32_t layer_begin, int32_t layer_end, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * scd_patch without a caller workspace and without any allocation: for callers that cannot call
+ * cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The same
+ * operation as scd_patch (Eq. 11, 12a/b), the same kernels; the intermediates
+ * (aligner activations a [T, d_a], u [T, d_model], sum-of-squares partials) live in a file-scope
+ * `static __device__` array of SCD_PATCH_STATIC_WORKSPACE_BYTES inside the library, which every GPU that
+ * loads the library holds until the process exits.  The caller passes inputs and outputs only.
+ *   - Limit: one PATCH layer's intermediates of the batch must fit: scd_plan_query's workspace for ONE layer,
+ *     about total_tokens * (d_aligner + d_model) * sizeof(state) bytes (32 MiB = ~2000 tokens at d_model 4096
+ *     in bf16).  Larger batches return SCD_E_WORKSPACE with the sizes in scd_last_error(); nothing is
+ *     enqueued.  Layers are grouped per launch by what the array holds, exactly as scd_patch does with a
+ *     small caller workspace (bit-identical results).
+ *   - The plan's device must be the current device.
+ *   - Calls no cudaMalloc / cudaFree / allocating library routine (the array's device address is looked up once
+ *     per device with cudaGetSymbolAddress).  Enqueues on `stream` and returns, like scd_patch.
+ *   - ALL calls on a device share the one array, which keeps the previous call's contents.  Nothing in it has to
+ *     start at zero (every byte a call reads was written earlier by the same call), so nothing is cleared; but two
+ *     calls that overlap on the GPU (different streams, no ordering between them) RACE on it -- serialise them,
+ *     or use scd_patch with separate workspaces. */
+#define SCD_PATCH_STATIC_WORKSPACE_BYTES (32u << 20)
+scd_status_t scd_patch_static(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
+                              const scd_paged_kv_t* kv, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Group-wise INT4 KV codec -- the paper's fastest transport baseline ("Quantized KV: transmits 4-bit
  * quantized KV caches (group-wise INT4) and dequantizes on the consumer"; Table 4
  * :352-359), built as the same-box comparison codec.  The paper fixes neither group

@@ -32,7 +32,7 @@ NO_SCALE = C.c_size_t(-1).value
 # every symbol include/scd.h declares
 EXPORTS = ["scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
            "scd_encode", "scd_reuse_decode", "scd_patch", "scd_encode_layers", "scd_reuse_decode_layers",
-           "scd_patch_layers", "scd_last_launch_count", "scd_profile_enable",
+           "scd_patch_layers", "scd_patch_static", "scd_last_launch_count", "scd_profile_enable",
            "scd_profile_fetch", "scd_last_error", "scd_version",
            "scd_int4_layout", "scd_int4_quantize", "scd_int4_dequantize_paged",
            "scd_fit_query", "scd_fit_reuse", "scd_struct_size"]
@@ -109,6 +109,8 @@ def _load() -> C.CDLL:
     lib.scd_encode_layers.argtypes = [vp, C.POINTER(BatchDesc), C.POINTER(SrcDesc), vp, i32, i32, vp]
     lib.scd_reuse_decode_layers.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), i32, i32, vp]
     lib.scd_patch_layers.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), vp, sz, i32, i32, vp]
+    lib.scd_patch_static.argtypes = [vp, C.POINTER(BatchDesc), vp, C.POINTER(PagedKV), vp]
+    lib.scd_patch_static.restype = C.c_int
     for name in ("scd_plan", "scd_plan_destroy", "scd_plan_query", "scd_plan_code_segment", "scd_code_layout",
                  "scd_encode", "scd_reuse_decode", "scd_patch"):
         getattr(lib, name).restype = C.c_int
@@ -285,6 +287,18 @@ def scd_reuse_decode(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: 
     else:
         _check(lib.scd_reuse_decode_layers(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), layers[0], layers[1],
                                            _stream_ptr(stream)))
+    return lib.scd_last_launch_count()
+
+
+PATCH_STATIC_WORKSPACE_BYTES = 32 << 20        # SCD_PATCH_STATIC_WORKSPACE_BYTES (include/scd.h)
+
+
+def scd_patch_static(plan: Plan, batch: BatchDesc, codes: torch.Tensor, k_pool: Sequence[Optional[torch.Tensor]],
+                     v_pool: Sequence[Optional[torch.Tensor]], n_blocks: int, stream=None, k_scale=None, v_scale=None) -> int:
+    """scd_patch with its intermediates in the library's static device array: no workspace argument, no allocation;
+    calls that overlap on the GPU race on that array (include/scd.h)."""
+    kv = _paged_kv(k_pool, v_pool, n_blocks, k_scale, v_scale)
+    _check(lib.scd_patch_static(plan.handle, C.byref(batch), _ptr(codes), C.byref(kv), _stream_ptr(stream)))
     return lib.scd_last_launch_count()
 
 

@@ -1,6 +1,7 @@
 // Host side of the C ABI (include/scd.h): validation, the static routing table and
 // artifact store (scd_plan), code-buffer layout, and the launch logic of the three hot
 // calls.  No arithmetic of the method happens on the host.
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -755,4 +756,50 @@ scd_status_t scd_patch_layers(const scd_plan_t* plan, const scd_batch_t* batch, 
   return scd_patch(plan, batch, codes, kv, workspace, workspace_bytes, stream);
 }
 
-}  // extern "C"
+// ---------------------------------------------------------------------------------
+// scd_patch_static: scd_patch with its intermediates in a static device array (no allocation, no caller workspace)
+// ---------------------------------------------------------------------------------
+}  // extern "C"  (the array and its address cache have internal linkage)
+
+// In HOST code this name is a host-side stand-in, not a device address: it is only ever handed to
+// cudaGetSymbolAddress below, never to a kernel.
+static __device__ __align__(256) unsigned char g_patch_static_ws[SCD_PATCH_STATIC_WORKSPACE_BYTES];
+
+// Device address of the array on `device`, looked up once per device with that device current.
+static scd_status_t patch_static_ws(int device, void** out) {
+  static std::atomic<void*> addr[scd::SCD_MAX_DEVICES];
+  if (device < 0 || device >= scd::SCD_MAX_DEVICES) return scd::fail(SCD_E_UNSUPPORTED, "scd_patch_static: device ordinal %d", device);
+  int cur = -1;
+  cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return scd::fail(SCD_E_CUDA, "scd_patch_static: cudaGetDevice: %s", cudaGetErrorString(e));
+  if (cur != device)
+    return scd::fail(SCD_E_ARG, "scd_patch_static: the plan lives on device %d but device %d is current", device, cur);
+  void* ptr = addr[device].load(std::memory_order_acquire);
+  if (!ptr) {
+    e = cudaGetSymbolAddress(&ptr, g_patch_static_ws);
+    if (e != cudaSuccess || !ptr)
+      return scd::fail(SCD_E_CUDA, "scd_patch_static: cudaGetSymbolAddress(static workspace): %s", cudaGetErrorString(e));
+    addr[device].store(ptr, std::memory_order_release);      // racing threads look up the same address
+  }
+  *out = ptr;
+  return SCD_OK;
+}
+
+extern "C" scd_status_t scd_patch_static(const scd_plan_t* plan, const scd_batch_t* batch, const void* codes,
+                                         const scd_paged_kv_t* kv, void* stream) {
+  using namespace scd;
+  reset_launch_count();
+  scd_status_t st = check_batch(plan, batch, true);
+  if (st != SCD_OK) return st;
+  if (batch->n_seqs == 0 || batch->total_tokens == 0 || plan->patches.empty()) return SCD_OK;
+  const PatchWs pw = patch_ws(plan, batch->total_tokens);
+  const size_t per_layer = pw.act_stride + pw.u_stride + pw.ss_stride;
+  if (per_layer > (size_t)SCD_PATCH_STATIC_WORKSPACE_BYTES)
+    return fail(SCD_E_WORKSPACE,
+                "scd_patch_static: one PATCH layer of %d tokens needs %zu bytes of intermediates, the static array holds %zu "
+                "(SCD_PATCH_STATIC_WORKSPACE_BYTES); use scd_patch with a caller workspace",
+                batch->total_tokens, per_layer, (size_t)SCD_PATCH_STATIC_WORKSPACE_BYTES);
+  void* ws = nullptr;
+  if ((st = patch_static_ws(plan->device, &ws)) != SCD_OK) return st;
+  return scd_patch(plan, batch, codes, kv, ws, (size_t)SCD_PATCH_STATIC_WORKSPACE_BYTES, stream);
+}
