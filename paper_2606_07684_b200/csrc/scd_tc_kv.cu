@@ -52,12 +52,18 @@ size_t kv_smem_bytes(int stages) {
   return 1024 + (size_t)stages * (A_STAGE_BYTES + KV_B_STAGE_BYTES) + KV_STG_BYTES + KV_VEC_BYTES + KV_SLOT_BYTES + sizeof(KvBarriers);
 }
 // ARES (code tile resident across the n-tiles of its (m-tile, segment)): num_kb slots of 16 KB + a ring of basis stages
+// Its shared memory is laid out tightly so that K = 256 gets a THIRD basis stage (two left main loop and epilogue adding up
+// instead of overlapping: 0.88 + 1.06 -> 1.68 ms on config 4): the small regions come first -- barriers (<= 512 B), ONE slot
+// table per lane quadrant (4 x 128 B) and the mean slices per column group, double-buffered by accumulator (4 x 2 x 256 B),
+// 3 KB in all instead of 6.4 KB of per-warp copies -- then the 1024-byte-aligned tiles.  With the dynamic shared memory
+// starting on a 1024-byte boundary (the kernel checks, and traps otherwise) that is exactly 227 KB at K = 256, three stages.
+constexpr int KVA_SMALL_BYTES = 3072, KVA_SLOT_OFF = 512, KVA_VEC_OFF = 1024;
+static_assert(sizeof(KvBarriers) <= KVA_SLOT_OFF, "barriers outgrew their 512 bytes");
 size_t kva_smem_bytes(int b_stages, int num_kb) {
-  return 1024 + (size_t)num_kb * A_STAGE_BYTES + (size_t)b_stages * KV_B_STAGE_BYTES + KV_STG_BYTES + KV_VEC_BYTES + KV_SLOT_BYTES +
-         sizeof(KvBarriers);
+  return KVA_SMALL_BYTES + (size_t)num_kb * A_STAGE_BYTES + (size_t)b_stages * KV_B_STAGE_BYTES + KV_STG_BYTES;
 }
 int kva_pick_stages(int num_kb) {
-  const size_t budget = 232448 - 1024 - KV_STG_BYTES - KV_VEC_BYTES - KV_SLOT_BYTES - sizeof(KvBarriers) - (size_t)num_kb * A_STAGE_BYTES;
+  const size_t budget = 232448 - KVA_SMALL_BYTES - KV_STG_BYTES - (size_t)num_kb * A_STAGE_BYTES;
   int st = (int)(budget / KV_B_STAGE_BYTES);
   return st > MAX_STAGES ? MAX_STAGES : st;
 }
@@ -159,14 +165,21 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
   static_assert(!ARES || AE4, "resident code tiles: e4m3 codes only");
   static_assert(!P8 || SCALED, "fp8 pools are built on the scaled variants only");
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  // ARES: small regions first, then the aligned tiles (see kva_smem_bytes)
+  uint8_t* smem = ARES ? (uint8_t*)(((uintptr_t)smem_raw + KVA_SMALL_BYTES + 1023) & ~(uintptr_t)1023)
+                       : (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   const int STAGES = P.stages;
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + (ARES ? P.num_kb : STAGES) * A_STAGE_BYTES;      // ARES: STAGES counts basis stages only
   uint8_t* smem_stg = smem_b + STAGES * KV_B_STAGE_BYTES;
-  uint8_t* smem_vec = smem_stg + KV_STG_BYTES;
-  uint8_t* smem_slot = smem_vec + KV_VEC_BYTES;
-  KvBarriers* bars = (KvBarriers*)(smem_slot + KV_SLOT_BYTES);
+  uint8_t* smem_vec = ARES ? smem_raw + KVA_VEC_OFF : smem_stg + KV_STG_BYTES;
+  uint8_t* smem_slot = ARES ? smem_raw + KVA_SLOT_OFF : smem_vec + KV_VEC_BYTES;
+  KvBarriers* bars = ARES ? (KvBarriers*)smem_raw : (KvBarriers*)(smem_slot + KV_SLOT_BYTES);
+  if (ARES) {
+    uint32_t dyn;
+    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+    if (smem_stg + KV_STG_BYTES > smem_raw + dyn) __trap();                 // the dynamic window did not start 1024-aligned
+  }
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.m_tiles * P.n_segs * P.n_tiles;
@@ -440,10 +453,15 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
     const int q = warp & 3;                                   // TMEM lane quadrant this warp may read
     const int g = (warp - KV_FIRST_EPI_WARP) >> 2;            // frequency / column group 0..3
     const uint32_t stg = ptx::smem_u32(smem_stg) + (uint32_t)q * (32 * KV_ROW_PITCH);
-    const uint32_t wvec = ptx::smem_u32(smem_vec) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 256;
+    // ARES: one slice per column group g (the four quadrants' warps write identical bytes), two buffers picked by the tile's
+    // accumulator; else one private slice per warp
+    const uint32_t wvec = ARES ? ptx::smem_u32(smem_vec) + (uint32_t)g * 512 : ptx::smem_u32(smem_vec) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 256;
     // the quadrant's 32 slot numbers, one private copy per warp (no cross-warp ordering needed): the copy-out reads the
     // slot of the row it stores with one broadcast LDS instead of shuffling a 64-bit address out of the owning lane
-    const uint32_t wslot = ptx::smem_u32(smem_slot) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 128;
+    // (ARES: one table per quadrant, written by its four warps -- identical values -- between the tile's two quadrant barriers)
+    const uint32_t wslot = ARES ? ptx::smem_u32(smem_slot) + (uint32_t)q * 128 : ptx::smem_u32(smem_slot) + (uint32_t)(warp - KV_FIRST_EPI_WARP) * 128;
+    int slot_reg = -1;
+    bool slot_dirty = false;
     const uint32_t bar_id = 1 + q;
     const uint32_t row_stride = (uint32_t)P.pool_width * (P8 ? 1u : 2u);  // bytes per slot
     // this lane's float4 of the warp's mean / bias slice: tile column for K tiles (runs a | b of both heads) / V tiles
@@ -519,9 +537,14 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
             rs_row = rsqrtf(ss / (float)P.rms_dim + P.rms_eps);
           }
         }
-        __syncwarp();
-        asm volatile("st.shared.b32 [%0], %1;" ::"r"(wslot + lane * 4), "r"((int)slot) : "memory");
-        __syncwarp();
+        if (ARES) {                                             // written once the previous tile's copy-out has drained
+          slot_reg = (int)slot;
+          slot_dirty = true;
+        } else {
+          __syncwarp();
+          asm volatile("st.shared.b32 [%0], %1;" ::"r"(wslot + lane * 4), "r"((int)slot) : "memory");
+          __syncwarp();
+        }
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
           const float2 x = rope_cs(pos, P.rope_g[16 * g + 2 * i]), y = rope_cs(pos, P.rope_g[16 * g + 2 * i + 1]);
@@ -541,15 +564,26 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
       if (P8) scale_base = (to1 ? sg.scale1 : sg.scale0) + ((to1 ? n0 - P.split : n0) >> 7) + ((lane >> 3) & 1);
       const uint32_t scale_stride = (uint32_t)(P.pool_width >> 7);
 
-      // this warp's slice of the tile's mean / bias: wvec[16 * run + i]
-      __syncwarp();
-      if (lane < 16)
-        asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wvec + lane * 16), "f"(cur.vec.x), "f"(cur.vec.y),
-                     "f"(cur.vec.z), "f"(cur.vec.w) : "memory");
-      __syncwarp();
+      // this warp's slice of the tile's mean / bias: wv[16 * run + i].  ARES: the slice is shared by the column group's four
+      // warps and written AFTER the accumulator has arrived -- by then every quadrant has handed back the tile before last,
+      // the previous user of this buffer
+      const uint32_t wv = ARES ? wvec + (uint32_t)acc * 256 : wvec;
+      if (!ARES) {
+        __syncwarp();
+        if (lane < 16)
+          asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wv + lane * 16), "f"(cur.vec.x), "f"(cur.vec.y),
+                       "f"(cur.vec.z), "f"(cur.vec.w) : "memory");
+        __syncwarp();
+      }
 
       ptx::mbar_wait_suspend(&bars->tmem_full[acc], acc_phase);
       ptx::tc_fence_after();
+      if (ARES) {
+        if (lane < 16)
+          asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(wv + lane * 16), "f"(cur.vec.x), "f"(cur.vec.y),
+                       "f"(cur.vec.z), "f"(cur.vec.w) : "memory");
+        __syncwarp();
+      }
       const uint32_t t_row = tmem_base + (uint32_t)(acc * KV_BLOCK_N) + ((uint32_t)(q * 32) << 16);
 
       Pre nxt = cur;
@@ -568,8 +602,8 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
           uint32_t oa[4], ob[4];
 #pragma unroll
           for (int q4 = 0; q4 < 2; ++q4) {
-            const float4 ma = ptx::lds_f4(wvec + ((2 * h) * 16 + 8 * hf + q4 * 4) * 4);
-            const float4 mb = ptx::lds_f4(wvec + ((2 * h + 1) * 16 + 8 * hf + q4 * 4) * 4);
+            const float4 ma = ptx::lds_f4(wv + ((2 * h) * 16 + 8 * hf + q4 * 4) * 4);
+            const float4 mb = ptx::lds_f4(wv + ((2 * h + 1) * 16 + 8 * hf + q4 * 4) * 4);
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
               const int i = q4 * 4 + e * 2, k = q4 * 2 + e, kf = 4 * hf + k;
@@ -587,7 +621,13 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
               ob[k] = pack_bf16x2(y0, y1);
             }
           }
-          if (hh == 0) ptx::named_bar_sync(bar_id, 128);        // the quadrant's previous copy-out has drained
+          if (hh == 0) {
+            ptx::named_bar_sync(bar_id, 128);                   // the quadrant's previous copy-out has drained
+            if (ARES && slot_dirty) {
+              asm volatile("st.shared.b32 [%0], %1;" ::"r"(wslot + lane * 4), "r"(slot_reg) : "memory");
+              slot_dirty = false;
+            }
+          }
           const int k0 = h * 16 + 2 * g + hf;                   // 16-B chunk of run (h, a); run (h, b) = +8
           ptx::sts128(qstg_addr(stg, lane, k0), make_uint4(oa[0], oa[1], oa[2], oa[3]));
           ptx::sts128(qstg_addr(stg, lane, k0 + 8), make_uint4(ob[0], ob[1], ob[2], ob[3]));
@@ -603,7 +643,7 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
           uint32_t o[8];
 #pragma unroll
           for (int q4 = 0; q4 < 4; ++q4) {
-            const float4 m4 = ptx::lds_f4(wvec + (c * 16 + q4 * 4) * 4);
+            const float4 m4 = ptx::lds_f4(wv + (c * 16 + q4 * 4) * 4);
             float v0, v1, v2, v3;
             const unsigned long long r01 = f2_pack(__uint_as_float(r[q4 * 4]), __uint_as_float(r[q4 * 4 + 1]));
             const unsigned long long r23 = f2_pack(__uint_as_float(r[q4 * 4 + 2]), __uint_as_float(r[q4 * 4 + 3]));
@@ -612,7 +652,13 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
             o[q4 * 2] = pack_bf16x2(v0, v1);
             o[q4 * 2 + 1] = pack_bf16x2(v2, v3);
           }
-          if (c == 0) ptx::named_bar_sync(bar_id, 128);
+          if (c == 0) {
+            ptx::named_bar_sync(bar_id, 128);
+            if (ARES && slot_dirty) {
+              asm volatile("st.shared.b32 [%0], %1;" ::"r"(wslot + lane * 4), "r"(slot_reg) : "memory");
+              slot_dirty = false;
+            }
+          }
           const int k0 = 8 * g + 2 * c;
           ptx::sts128(qstg_addr(stg, lane, k0), make_uint4(o[0], o[1], o[2], o[3]));
           ptx::sts128(qstg_addr(stg, lane, k0 + 1), make_uint4(o[4], o[5], o[6], o[7]));
