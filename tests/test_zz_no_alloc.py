@@ -99,3 +99,27 @@ def test_patch_static_refuses_batches_beyond_its_array(cuda_device):
     # the same batch goes through scd_patch with a caller workspace
     assert B.scd_patch(prob.plan, prob.bdesc, prob.codes, k8, v8, prob.batch.n_blocks, prob.workspace) > 0
     torch.cuda.synchronize()
+
+
+def test_patch_static_on_the_fp32_path(cuda_device):
+    """Tiny (fp32 states, SIMT kernels): the static array serves that path too; pools must equal scd_patch's bit for bit."""
+    from paper_2606_07684_b200 import binding as B
+    from paper_2606_07684_b200.harness import CodecProblem
+    prob = CodecProblem(W.CONFIGS["tiny"], cuda_device)
+    k, v, h = prob.make_sources()
+    prob.alloc_pools()
+    prob.encode(k, v, h)
+    nb, L = prob.batch.n_blocks, prob.cfg.n_layers
+    ref_k = [torch.full_like(p, float("nan")) for p in prob.k_pool]
+    ref_v = [torch.full_like(p, float("nan")) for p in prob.v_pool]
+    new_k = [t.clone() for t in ref_k]
+    new_v = [t.clone() for t in ref_v]
+    B.scd_patch(prob.plan, prob.bdesc, prob.codes, ref_k, ref_v, nb, prob.workspace)
+    B.scd_patch_static(prob.plan, prob.bdesc, prob.codes, new_k, new_v, nb)
+    torch.cuda.synchronize()
+    wrote = False
+    for l in range(L):
+        for got, want in ((new_k[l], ref_k[l]), (new_v[l], ref_v[l])):
+            assert torch.equal(got.view(torch.int32), want.view(torch.int32)), f"layer {l}"
+            wrote |= bool(torch.isfinite(want).any())
+    assert wrote
