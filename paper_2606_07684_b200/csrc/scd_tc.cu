@@ -1626,6 +1626,9 @@ scd_status_t tc_reuse_decode(const scd_plan_t* p, const scd_batch_t* batch, cons
     if (P.pool_e4m3 && !tc_kv_eligible(p, P)) return fail(SCD_E_UNSUPPORTED, "fp8 pools: D must be a multiple of 256");
     // the paged-KV kernel takes 256-column tiles of 128-wide heads (e4m3 codes: widened in shared memory by its own
     // warps); anything else runs on the generic kernel
+    // a call with more than TC_MAX_SEGS (layer, branch) segments takes several launches over disjoint layers: like the
+    // encode's, they overlap at their seams (dep_wait_late)
+    P.dep_wait_late = (TC_ENC_OVERLAP && i > 0) ? 1 : 0;
     if (tc_kv_eligible(p, P)) st = launch_tc_kv(p, P, s);
     else st = e4 ? launch_tc<EPI_KV, A_CODES>(p, P, s) : launch_tc<EPI_KV, A_PLAIN>(p, P, s);
     if (st != SCD_OK) return st;
@@ -1654,6 +1657,7 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
   if (group < 1) group = 1;
   if (group > TC_MAX_SEGS) group = TC_MAX_SEGS;
   size_t j0 = 0;
+  int n_groups_done = 0;
   while (j0 < p->patches.size()) {
     if (!layer_in_window(p->patches[j0].layer)) { ++j0; continue; }
     size_t j1 = j0;
@@ -1678,6 +1682,10 @@ scd_status_t tc_patch(const scd_plan_t* p, const scd_batch_t* batch, const void*
       sg.a_scale = e4 ? (const float*)((const char*)codes + soff[key]) : nullptr;
     }
     P.prof_id = SCD_PROF_PATCH_GEMM1;
+    // a later group's GEMM-1 reads codes and overwrites activation slices whose reader (the previous group's GEMM-2) completed
+    // before that group's GEMM-3 started: independent of its stream predecessor, the previous group's GEMM-3 (dep_wait_late)
+    P.dep_wait_late = (TC_ENC_OVERLAP && n_groups_done > 0) ? 1 : 0;
+    ++n_groups_done;
     if ((st = e4 ? launch_tc<EPI_ACT, A_CODES>(p, P, s) : launch_tc<EPI_ACT, A_PLAIN>(p, P, s)) != SCD_OK) return st;
     // GEMM-2: [T, d_a] x [d_a, d] per layer
     fill_common(p, batch, true, false, P);

@@ -53,7 +53,7 @@ struct TcParams {
   int32_t pool_e4m3;                  // paged-KV kernel: pools are e4m3 bytes + per-(slot, head) fp32 scales
   int32_t pair;                       // generic kernel, host only: launch as CTA pairs (cta_group::2), B maps have 128-row boxes
   int32_t a_gather;                   // generic kernel: A rows are gathered through P.batch.page_table (paged producer cache)
-  int32_t dep_wait_late;              // generic kernel: this launch reads nothing its stream predecessor writes (see tc_encode)
+  int32_t dep_wait_late;              // both kernels: this launch reads nothing its stream predecessor writes (see tc_encode)
   int32_t b_res;                      // generic kernel, PATCH GEMM-1: the B tile stays resident across a CTA's consecutive m-tiles
   long long pool_slots;               // paged epilogues: n_blocks * block_size (slot numbers are kept as int32)
 };

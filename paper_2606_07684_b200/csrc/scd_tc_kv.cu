@@ -216,7 +216,9 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
   __syncthreads();
   ptx::tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
-  ptx::grid_dep_wait();                 // the previous kernel of the stream has completed and flushed
+  // the previous kernel of the stream has completed and flushed (P.dep_wait_late: a later launch of one scd_reuse_decode
+  // call, independent of its predecessor -- it waits at its END instead, see tc_gemm_kernel)
+  if (!P.dep_wait_late) ptx::grid_dep_wait();
   ptx::grid_dep_launch_dependents();    // the next one may start its prologue as SMs free up
 
   if (warp < KV_FIRST_EPI_WARP) {
@@ -718,6 +720,7 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
 
   // ============================== teardown ==============================
   ptx::tc_fence_before();
+  if (P.dep_wait_late && threadIdx.x == 0) ptx::grid_dep_wait();
   __syncthreads();
   if (warp == 0) ptx::tmem_dealloc<TMEM_COLS>(tmem_base);
 }
