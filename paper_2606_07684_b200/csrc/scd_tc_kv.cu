@@ -22,6 +22,9 @@
 #ifndef KV_ARES
 #define KV_ARES 1
 #endif
+#ifndef KV_ARES_BF16
+#define KV_ARES_BF16 1
+#endif
 #ifndef KV_STATIC_PCT
 #define KV_STATIC_PCT 60
 #endif
@@ -162,7 +165,7 @@ constexpr int KV_NTHREADS_E4 = KV_NTHREADS + KV_XF_WARPS * 32;          // 896
 template <bool DYN, bool SCALED, bool AE4, bool P8, bool ARES = false>
 __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_kernel(const __grid_constant__ TcParams P) {
   static_assert(!AE4 || (SCALED && !DYN), "e4m3 codes carry row scales; static split");
-  static_assert(!ARES || AE4, "resident code tiles: e4m3 codes only");
+  static_assert(!ARES || !DYN, "resident code tiles: static split (REUSE decode)");
   static_assert(!P8 || SCALED, "fp8 pools are built on the scaled variants only");
   extern __shared__ uint8_t smem_raw[];
   // ARES: small regions first, then the aligned tiles (see kva_smem_bytes)
@@ -246,8 +249,9 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
           for (int kb = 0; kb < P.num_kb; ++kb) {
             if (grp_first) {                                   // the code tile's k-block, once its slot has been released
               if (groups > 0) ptx::mbar_wait_suspend(&bars->a_empty[kb], (groups - 1) & 1);
-              ptx::mbar_expect_tx(&bars->a_full[kb], A_STAGE_BYTES / 2);
-              ptx::tma_load_3d(smem_a + kb * A_STAGE_BYTES + A_STAGE_BYTES / 2, &P.a_maps[sg.a_map], &bars->a_full[kb], kb * BLOCK_K,
+              // e4m3 codes: the raw tile lands in the upper half of its slot and is widened in place; bf16 codes: the slot itself
+              ptx::mbar_expect_tx(&bars->a_full[kb], AE4 ? A_STAGE_BYTES / 2 : A_STAGE_BYTES);
+              ptx::tma_load_3d(smem_a + kb * A_STAGE_BYTES + (AE4 ? A_STAGE_BYTES / 2 : 0), &P.a_maps[sg.a_map], &bars->a_full[kb], kb * BLOCK_K,
                                tc.m_tile * BLOCK_M, sg.a_z);
             }
             ptx::mbar_wait_suspend(&bars->empty[stage], phase ^ 1);
@@ -335,7 +339,7 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
           ptx::tc_fence_after();
           const uint32_t d_tmem = tmem_base + (uint32_t)(acc * KV_BLOCK_N);
           for (int kb = 0; kb < P.num_kb; ++kb) {
-            if (grp_first) ptx::mbar_wait_suspend(&bars->a_ready[kb], groups & 1);      // landed and widened, once per group
+            if (grp_first) ptx::mbar_wait_suspend(AE4 ? &bars->a_ready[kb] : &bars->a_full[kb], groups & 1);   // landed (and widened), once per group
             ptx::mbar_wait_suspend(&bars->full[stage], phase);
             ptx::tc_fence_after();
             const uint64_t da = ptx::umma_desc_sw128(ptx::smem_u32(smem_a + kb * A_STAGE_BYTES));
@@ -756,6 +760,34 @@ scd_status_t launch_tc_kv(const scd_plan_t* p, TcParams& P, cudaStream_t s) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(tc_kv_kernel<false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv smem %zu): %s", smem, cudaGetErrorString(e));
     configured[p->device].store(smem, std::memory_order_relaxed);
+  }
+  // bf16 codes on bf16 pools, plain REUSE decode (no row scales): resident code tile as well -- the ring then holds basis tiles
+  // only and a code tile leaves L2 once per (m-tile, segment) instead of once per n-tile.  Measured on config-2 geometry
+  // (profiles/r02_decode_history.md section 17): faster at one k-block per tile (r <= 64: four tiles' basis in flight instead of two
+  // whole stages; config 3 0.508 -> 0.469 ms) and at three or four (r = 192, 256: +1-2 %), slower at two (r = 96, 128: -4 %,
+  // where three 48 KB stages already hold 1.5 tiles) -- so two k-blocks keep the plain kernel
+  {
+    bool any_scale = false;
+    for (int i = 0; i < P.n_segs; ++i) any_scale |= P.segs[i].rowscale_in != nullptr || P.segs[i].a_scale != nullptr;
+    if (KV_ARES_BF16 && P.code_dtype == SCD_BF16 && P.a_is_codes && !any_scale && !P.pool_e4m3 && P.head_rank == 0 && P.num_kb <= 4 &&
+        P.num_kb != 2 && P.n_tiles > 1) {
+      P.stages = kva_pick_stages(P.num_kb);
+      const size_t smem_b_ = kva_smem_bytes(P.stages, P.num_kb);
+      static std::atomic<size_t> conf_b[SCD_MAX_DEVICES];
+      if (conf_b[p->device].load(std::memory_order_relaxed) < smem_b_) {
+        cudaError_t e = cudaFuncSetAttribute(tc_kv_kernel<false, false, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b_);
+        if (e != cudaSuccess) return fail(SCD_E_CUDA, "cudaFuncSetAttribute(kv resident bf16 smem %zu): %s", smem_b_, cudaGetErrorString(e));
+        conf_b[p->device].store(smem_b_, std::memory_order_relaxed);
+      }
+      if ((long long)P.pool_slots >= (1ll << 31)) return fail(SCD_E_UNSUPPORTED, "pools of more than 2^31 slots");
+      prof_begin(s);
+      launch_pdl(tc_kv_kernel<false, false, false, false, true>, std::min(total, p->sm_count), KV_NTHREADS, smem_b_, s, 1, P);
+      prof_end(s, P.prof_id);
+      cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) return fail(SCD_E_CUDA, "tc_kv_kernel (resident bf16 code tile) launch: %s", cudaGetErrorString(e));
+      count_launch();
+      return SCD_OK;
+    }
   }
   // e4m3 codes of rank <= 256 on bf16 pools: the code tile stays resident across its n-tiles
   if (KV_ARES && P.code_dtype == SCD_E4M3_ROWSCALE && P.a_is_codes && !P.pool_e4m3 && P.head_rank == 0 && P.num_kb <= 4 && P.n_tiles > 1) {

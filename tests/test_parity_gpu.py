@@ -470,6 +470,18 @@ def test_e4m3_decode_with_several_tiles_per_cta(rank, cuda_device):
     print(rank, res)
 
 
+@pytest.mark.parametrize("rank", [32, 64, 192, 256])
+def test_bf16_decode_with_a_resident_code_tile_and_several_tiles_per_cta(rank, cuda_device):
+    """bf16 codes with one, three or four k-blocks per tile decode on the resident-code-tile variant too (two k-blocks keep
+    the plain kernel).  Same geometry as the e4m3 case above: 504 tiles on 148 CTAs, groups entered and left mid-way, the slot
+    table shared per lane quadrant and the mean slices shared per column group, ragged requests, permuted pages."""
+    cfg = MINI["llama3_8b_8k"].scaled(n_layers=4, patch_layers=(3,), seqlens=(1500, 1100, 7), d_model=512, rank=rank,
+                                      permute_pages=True)
+    prob = _problem(cfg, cuda_device, pos_offset=[0, 40, 3])
+    res = _run_all(prob)
+    print(rank, res)
+
+
 def test_patch_gemms_on_cta_pairs_with_several_tiles_per_pair(cuda_device):
     """PATCH GEMM-2 / GEMM-3 run as CTA pairs (tcgen05 cta_group::2).  39 m-tiles (odd: the last pair has an out-of-range
     partner) x 4 n-tiles x 2 layers = 160 / 320 pair tiles on 74 pairs: every pair walks several tiles, through the L2
