@@ -471,16 +471,34 @@ def run_ours(args, cfg):
         # pools device -> host.  Inputs and pools are double-buffered and the copies run on their own streams, so
         # step i's D2H and step i+1's H2D overlap (PCIe is full duplex) with step i+1's compute waiting only on
         # its own inputs; every step's copies are inside the timed region.
-        sets = [{"k": k, "v": v, "h": h, "kp": prob.k_pool, "vp": prob.v_pool}]
-        clone = lambda ts: [None if t is None else t.clone() for t in ts]
-        sets.append({"k": clone(k), "v": clone(v), "h": clone(h), "kp": clone(prob.k_pool), "vp": clone(prob.v_pool)})
-        for st in sets:
-            st["srcs"] = [t for t in (st["k"] + st["v"] + st["h"]) if t is not None]
-            st["pools"] = list(st["kp"] + st["vp"])
-        host_in = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True).copy_(t) for t in sets[0]["srcs"]]
-        host_out = [torch.empty(p.shape, dtype=p.dtype, pin_memory=True) for p in sets[0]["pools"]]
-        h2d = sum(t.numel() * t.element_size() for t in sets[0]["srcs"])
-        d2h = sum(p.numel() * p.element_size() for p in sets[0]["pools"])
+        # The per-layer tensors the C ABI takes are views into ONE device slab per direction (and the host side is one
+        # pinned buffer per direction), so a step's transfer is one copy each way: 67 per-tensor copies each way reach
+        # 41.6 GB/s per direction on this box, one copy 50 GB/s (both directions busy).
+        def slab_views(ts):
+            nb = [0 if t is None else (t.numel() * t.element_size() + 255) // 256 * 256 for t in ts]
+            slab = torch.empty(sum(nb), dtype=torch.uint8, device=dev)
+            views, off = [], 0
+            for t, n in zip(ts, nb):
+                if t is None:
+                    views.append(None)
+                    continue
+                vw = slab[off:off + t.numel() * t.element_size()].view(t.dtype).view(t.shape)
+                vw.copy_(t)
+                views.append(vw)
+                off += n
+            return slab, views
+        sets = []
+        for _ in range(2):
+            src_slab, sv = slab_views(list(k) + list(v) + list(h))
+            pool_slab, pv = slab_views(list(prob.k_pool) + list(prob.v_pool))
+            L_ = len(k)
+            sets.append({"k": sv[:L_], "v": sv[L_:2 * L_], "h": sv[2 * L_:], "kp": pv[:len(prob.k_pool)], "vp": pv[len(prob.k_pool):],
+                         "src_slab": src_slab, "pool_slab": pool_slab})
+        host_in = torch.empty(sets[0]["src_slab"].shape, dtype=torch.uint8, pin_memory=True).copy_(sets[0]["src_slab"])
+        host_out = torch.empty(sets[0]["pool_slab"].shape, dtype=torch.uint8, pin_memory=True)
+        h2d = sum(t.numel() * t.element_size() for t in (list(k) + list(v) + list(h)) if t is not None)
+        d2h = sum(p.numel() * p.element_size() for p in (list(prob.k_pool) + list(prob.v_pool)) if p is not None)
+        orig_pools = (prob.k_pool, prob.v_pool)
         s_in, s_out = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev)
         in_done, comp_done, out_done = [ev(), ev()], [ev(), ev()], [ev(), ev()]
 
@@ -489,8 +507,7 @@ def run_ours(args, cfg):
             if i >= 2:
                 s_in.wait_event(comp_done[bi])            # step i-2 has consumed this input buffer
             with torch.cuda.stream(s_in):
-                for dst, src in zip(st["srcs"], host_in):
-                    dst.copy_(src, non_blocking=True)
+                st["src_slab"].copy_(host_in, non_blocking=True)
                 in_done[bi].record(s_in)
             stream.wait_event(in_done[bi])
             if i >= 2:
@@ -500,15 +517,14 @@ def run_ours(args, cfg):
             comp_done[bi].record(stream)
             s_out.wait_event(comp_done[bi])
             with torch.cuda.stream(s_out):
-                for dst, src in zip(host_out, st["pools"]):
-                    dst.copy_(src, non_blocking=True)
+                host_out.copy_(st["pool_slab"], non_blocking=True)
                 out_done[bi].record(s_out)
 
         e2e_step(0); e2e_step(1)
         torch.cuda.synchronize()
         barrier()
         a, b = ev(), ev()
-        n_e2e = max(4, min(args.steps, 10))
+        n_e2e = max(4, args.steps)                 # the same K steps as the device-timed region (pipeline fill and drain included)
         a.record(stream)
         for i in range(n_e2e):
             e2e_step(i + 2)
@@ -516,7 +532,8 @@ def run_ours(args, cfg):
         b.record(stream)
         barrier()
         e2e_ms = a.elapsed_time(b) / n_e2e
-        prob.k_pool, prob.v_pool = sets[0]["kp"], sets[0]["vp"]
+        prob.k_pool, prob.v_pool = orig_pools
+        del sets, host_in, host_out
         e2e = {"ms": e2e_ms, "h2d": h2d, "d2h": d2h}
     clocks = sampler.stop() if sampler else None
     extras = None
