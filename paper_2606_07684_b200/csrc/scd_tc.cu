@@ -38,6 +38,8 @@ struct __align__(8) TcBarriers {
   uint64_t full[MAX_STAGES], empty[MAX_STAGES], ready[MAX_STAGES];
   uint64_t tmem_full[2], tmem_empty[2];
   uint64_t b_full[4], b_empty[4];              // B-resident mode (PATCH GEMM-1): the resident B tile's k-block slots
+  uint64_t sched_full[4], sched_empty[4];      // dynamic tile claiming (plain encodes): ring of claimed tile ids
+  int32_t sched_tile[4];                       // -1 = no more tiles
   uint32_t tmem_base;
 };
 
@@ -373,6 +375,12 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
   const int t_begin = bres ? (int)((long long)blockIdx.x * total_tiles / gridDim.x) : walker;
   const int t_end = bres ? (int)((long long)(blockIdx.x + 1) * total_tiles / gridDim.x) : total_tiles;
   const int t_step = bres ? 1 : walk_stride;
+  // Dynamic tile claiming (the encode's plain launches, P.sched set by the host): every CTA starts on tile blockIdx.x and then
+  // claims tiles from a global counter (the producer thread, always one claim ahead of the tile it is loading) and hands
+  // them to the MMA thread and the epilogue warps through a four-entry ring.  A launch that starts while its predecessor's
+  // last wave is still running (dep_wait_late) then fills the hole that wave leaves: CTAs that start late claim fewer tiles.
+  constexpr bool DYN_OK = EPI == EPI_CODES && AMODE == A_PLAIN && !PAIR;
+  const bool dyn = DYN_OK && P.sched != nullptr;
 
   if (warp == 0 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) {
@@ -383,6 +391,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     for (int k = 0; k < 4; ++k) {
       ptx::mbar_init(&bars->b_full[k], 1);
       ptx::mbar_init(&bars->b_empty[k], 1);
+      ptx::mbar_init(&bars->sched_full[k], 1);
+      ptx::mbar_init(&bars->sched_empty[k], 1 + NEPI);           // MMA thread + one lane per epilogue warp
     }
     for (int a = 0; a < 2; ++a) {
       ptx::mbar_init(&bars->tmem_full[a], 1);
@@ -517,7 +527,21 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     if (lane == 0) {
       int stage = 0;
       uint32_t phase = 0;
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+      int sslot = 0;
+      uint32_t sphase = 0;
+      int tile = blockIdx.x;
+      int next = dyn ? (int)gridDim.x + atomicAdd(P.sched, 1) : tile + (int)gridDim.x;
+      for (;;) {
+        // dynamic: claim the tile after next now (the atomic's latency hides under this tile's loads), publish this one
+        int after = next + (int)gridDim.x;
+        if (dyn) {
+          after = next < total_tiles ? (int)gridDim.x + atomicAdd(P.sched, 1) : next;
+          ptx::mbar_wait_suspend(&bars->sched_empty[sslot], sphase ^ 1);
+          *(volatile int*)&bars->sched_tile[sslot] = tile < total_tiles ? tile : -1;
+          ptx::mbar_arrive(&bars->sched_full[sslot]);
+          if (++sslot == 4) { sslot = 0; sphase ^= 1; }
+        }
+        if (tile >= total_tiles) break;
         int m_tile, n_tile, seg_i;
         tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
         const TcSeg& sg = P.segs[seg_i];
@@ -527,8 +551,8 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
         // into L2 now, so that the few shared-memory stages see L2 latency instead of HBM latency
         const int pf = P.a_prefetch < P.num_kb ? P.a_prefetch : P.num_kb;
         int nm_tile = 0, nn_tile = 0, nseg_i = 0;
-        const bool has_next = tile + (int)gridDim.x < total_tiles;
-        if (pf > 0 && has_next) tile_decode(P, walk_mt, tile + gridDim.x, nm_tile, nn_tile, nseg_i);
+        const bool has_next = next < total_tiles;
+        if (pf > 0 && has_next) tile_decode(P, walk_mt, next, nm_tile, nn_tile, nseg_i);
         for (int kb = 0; kb < P.num_kb; ++kb) {
           if (pf > 0) {
             const bool same = kb + pf < P.num_kb;
@@ -556,6 +580,16 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
                              m_tile * BLOCK_M, sg.a_z);
           ptx::tma_load_2d(smem_b + stage * b_stage_bytes, bm, &bars->full[stage], kb * BLOCK_K, n_tile * block_n);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        tile = next;
+        next = after;
+      }
+      if (dyn) {                                  // the last CTA to stop claiming re-arms the counters for a later launch
+        __threadfence();
+        if (atomicAdd(P.sched + 1, 1) == (int)gridDim.x - 1) {
+          P.sched[0] = 0;
+          P.sched[1] = 0;
+          __threadfence();
         }
       }
     }
@@ -605,7 +639,16 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
       int stage = 0;
       uint32_t phase = 0;
       int it = 0;
-      for (int tile = walker; tile < total_tiles; tile += walk_stride, ++it) {
+      int sslot = 0;
+      uint32_t sphase = 0;
+      for (int tile = walker; dyn || tile < total_tiles; tile += walk_stride, ++it) {
+        if (dyn) {                                // the tile count is all this thread needs from the ring
+          ptx::mbar_wait_suspend(&bars->sched_full[sslot], sphase);
+          const int t = *(volatile int*)&bars->sched_tile[sslot];
+          ptx::mbar_arrive(&bars->sched_empty[sslot]);
+          if (++sslot == 4) { sslot = 0; sphase ^= 1; }
+          if (t < 0) break;
+        }
         const int acc = it & 1;
         const uint32_t acc_phase = (it >> 1) & 1;
         ptx::mbar_wait_suspend(&bars->tmem_empty[acc], acc_phase ^ 1);
@@ -741,8 +784,19 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
     } else {
     int it = 0;
     RowInfo cur;
-    if (t_begin < t_end) cur = fetch(t_begin);
-    for (int tile = t_begin; tile < t_end; tile += t_step, ++it) {
+    int sslot = 0;
+    uint32_t sphase = 0;
+    if (!dyn && t_begin < t_end) cur = fetch(t_begin);
+    for (int tile = t_begin; dyn || tile < t_end; tile += t_step, ++it) {
+      if (dyn) {                                  // claimed tiles arrive through the ring; no look-ahead on the next one
+        ptx::mbar_wait_suspend(&bars->sched_full[sslot], sphase);
+        tile = *(volatile int*)&bars->sched_tile[sslot];
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&bars->sched_empty[sslot]);
+        if (++sslot == 4) { sslot = 0; sphase ^= 1; }
+        if (tile < 0) break;
+        cur = fetch(tile);
+      }
       int m_tile, n_tile, seg_i;
       tile_decode(P, walk_mt, tile, m_tile, n_tile, seg_i);
       if (PAIR) m_tile = 2 * m_tile + (int)cta_rank;
@@ -782,7 +836,7 @@ tc_gemm_kernel(const __grid_constant__ TcParams P) {
 
       // prefetch the next tile's per-row quantities; consumed at the bottom of the loop
       RowInfo nxt = cur;
-      if (tile + t_step < t_end) nxt = fetch(tile + t_step);
+      if (!dyn && tile + t_step < t_end) nxt = fetch(tile + t_step);
 
       if (EPI == EPI_KV && n0 < sg.rope_cols && P.rope_style == SCD_ROPE_HALF && P.head_dim == 128 && block_n == 256 &&
           n_end == 256) {
@@ -1270,6 +1324,9 @@ static scd_status_t make_b_map(CUtensorMap* m, const void* base, int N, int K, i
 #ifndef TC_ENC_PAIRS
 #define TC_ENC_PAIRS 1
 #endif
+#ifndef TC_ENC_DYN
+#define TC_ENC_DYN 1
+#endif
 #ifndef TC_ENC_OVERLAP
 #define TC_ENC_OVERLAP 1
 #endif
@@ -1480,8 +1537,15 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
   size_t i = 0;
   int n_launched = 0;
   const size_t nseg = p->segs.size();
+  // Launch order K, H, V: the launches overlap at their seams (dep_wait_late) and the plain ones claim their tiles
+  // dynamically, so the V launch -- many short tiles -- goes last and fills the hole the H launch leaves (config 2: 192
+  // tiles of 64 k-blocks on 148 SMs, a second wave of 44)
+  // (measured on config 2 with dynamic claiming: K, H, V 0.257 ms; H, K, V 0.263 ms; K, V, H 0.291 ms)
+  static const int kPassBranch[3] = {SCD_BRANCH_K, SCD_BRANCH_H, SCD_BRANCH_V};
+  for (int pass = 0; pass < 3; ++pass) {
+  i = 0;
   while (i < nseg) {
-    if (!layer_in_window(p->segs[i].layer)) { ++i; continue; }
+    if (!layer_in_window(p->segs[i].layer) || p->segs[i].branch != kPassBranch[pass]) { ++i; continue; }
     // a launch = run of segments (inside the call's layer window) with the same branch, rank and width
     size_t j = i;
     // (a paged source needs two descriptors per segment: half as many segments per launch)
@@ -1549,10 +1613,13 @@ scd_status_t tc_encode(const scd_plan_t* p, const scd_batch_t* batch, const scd_
         P.pair = 1;
         for (size_t q = i; q < j; ++q) P.segs[q - i].b_map = 2 * (int)nseg + 5 * (int)p->patches.size() + p->segs[q].seg_index;
       }
+      if (TC_ENC_DYN && !P.pair && !gather)      // dynamic tile claiming: a plan-owned counter pair per launch in flight
+        P.sched = p->kv_sched + 2 * (p->kv_sched_next.fetch_add(1) % KV_SCHED_SETS);
       st = launch_tc<EPI_CODES, A_PLAIN>(p, P, s);
     }
     if (st != SCD_OK) return st;
     i = j;
+  }
   }
   return SCD_OK;
 }
