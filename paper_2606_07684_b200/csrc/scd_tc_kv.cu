@@ -63,7 +63,9 @@ size_t kv_smem_bytes(int stages) {
 constexpr int KVA_SMALL_BYTES = 3072, KVA_SLOT_OFF = 512, KVA_VEC_OFF = 1024;
 static_assert(sizeof(KvBarriers) <= KVA_SLOT_OFF, "barriers outgrew their 512 bytes");
 size_t kva_smem_bytes(int b_stages, int num_kb) {
-  return KVA_SMALL_BYTES + (size_t)num_kb * A_STAGE_BYTES + (size_t)b_stages * KV_B_STAGE_BYTES + KV_STG_BYTES;
+  const size_t need = KVA_SMALL_BYTES + (size_t)num_kb * A_STAGE_BYTES + (size_t)b_stages * KV_B_STAGE_BYTES + KV_STG_BYTES;
+  // wherever it costs no stage (every rank but 256), 1 KB of slack makes the carve-up independent of the window's alignment
+  return need + 1024 <= 232448 ? need + 1024 : need;
 }
 int kva_pick_stages(int num_kb) {
   const size_t budget = 232448 - KVA_SMALL_BYTES - KV_STG_BYTES - (size_t)num_kb * A_STAGE_BYTES;
