@@ -59,7 +59,8 @@ size_t kv_smem_bytes(int stages) {
 // instead of overlapping: 0.88 + 1.06 -> 1.68 ms on config 4): the small regions come first -- barriers (<= 512 B), ONE slot
 // table per lane quadrant (4 x 128 B) and the mean slices per column group, double-buffered by accumulator (4 x 2 x 256 B),
 // 3 KB in all instead of 6.4 KB of per-warp copies -- then the 1024-byte-aligned tiles.  With the dynamic shared memory
-// starting on a 1024-byte boundary (the kernel checks, and traps otherwise) that is exactly 227 KB at K = 256, three stages.
+// starting on a 1024-byte boundary (if it ever does not, the kernel runs with one stage less) that is exactly 227 KB at K = 256,
+// three stages.
 constexpr int KVA_SMALL_BYTES = 3072, KVA_SLOT_OFF = 512, KVA_VEC_OFF = 1024;
 static_assert(sizeof(KvBarriers) <= KVA_SLOT_OFF, "barriers outgrew their 512 bytes");
 size_t kva_smem_bytes(int b_stages, int num_kb) {
@@ -173,18 +174,23 @@ __global__ void __launch_bounds__(AE4 ? KV_NTHREADS_E4 : KV_NTHREADS, 1) tc_kv_k
   // ARES: small regions first, then the aligned tiles (see kva_smem_bytes)
   uint8_t* smem = ARES ? (uint8_t*)(((uintptr_t)smem_raw + KVA_SMALL_BYTES + 1023) & ~(uintptr_t)1023)
                        : (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  const int STAGES = P.stages;
+  int stages_fit = P.stages;
+  if (ARES) {
+    // The host sizes the window for tiles that start on a 1024-byte boundary right after the small regions.  Should the
+    // window itself not start on one, the ring gives up a stage instead of running past the end (every role takes the same
+    // decision from the same addresses).
+    uint32_t dyn;
+    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+    while (stages_fit > 1 && smem + (size_t)P.num_kb * A_STAGE_BYTES + (size_t)stages_fit * KV_B_STAGE_BYTES + KV_STG_BYTES > smem_raw + dyn)
+      --stages_fit;
+  }
+  const int STAGES = stages_fit;
   uint8_t* smem_a = smem;
   uint8_t* smem_b = smem + (ARES ? P.num_kb : STAGES) * A_STAGE_BYTES;      // ARES: STAGES counts basis stages only
   uint8_t* smem_stg = smem_b + STAGES * KV_B_STAGE_BYTES;
   uint8_t* smem_vec = ARES ? smem_raw + KVA_VEC_OFF : smem_stg + KV_STG_BYTES;
   uint8_t* smem_slot = ARES ? smem_raw + KVA_SLOT_OFF : smem_vec + KV_VEC_BYTES;
   KvBarriers* bars = ARES ? (KvBarriers*)smem_raw : (KvBarriers*)(smem_slot + KV_SLOT_BYTES);
-  if (ARES) {
-    uint32_t dyn;
-    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
-    if (smem_stg + KV_STG_BYTES > smem_raw + dyn) __trap();                 // the dynamic window did not start 1024-aligned
-  }
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int total_tiles = P.m_tiles * P.n_segs * P.n_tiles;
